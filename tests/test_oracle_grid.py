@@ -1,0 +1,349 @@
+"""Pins for the oracle's full VL+CT step.
+
+  T1  uniform magnetised state unchanged bit-for-bit (PLMC and PPMC)
+  T8  linear fast wave returns to its closed-form initial state, ~2nd order
+  T9  identical error along x, y, z and for the left-going wave
+  T10 div B at round-off, mass/momentum/energy conserved to round-off
+  T12 Brio & Wu planar invariants and plateau values
+  T13 blast: point symmetry, positivity
+  T14 B = 0: Sod shock tube against the textbook exact Riemann solution
+  plus Eq. 11 on states with a closed-form answer.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_2402_05240_b200 import inputs
+from helpers import run_to_time, run_steps, divb_normalised, totals, FIELDS
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def make(p):
+    o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc)
+    o.set_state(p.state)
+    return o
+
+
+@pytest.mark.parametrize("recon", [0, 1, 2])
+def test_T1_uniform_state_bit_for_bit(recon):
+    p = inputs.uniform(n=(8, 6, 5), recon=recon)
+    o = make(p)
+    dt = o.compute_dt(0.4)
+    for _ in range(3):
+        o.step(dt)
+    out = o.get_state()
+    for f in FIELDS:
+        assert np.array_equal(out[f], p.state[f]), f
+
+
+def test_compute_dt_closed_forms():
+    # Eq. 11-12 on a uniform state: B along x only ->
+    # c_f,x = max(a, c_A), c_f,y = c_f,z = sqrt(a^2 + c_A^2)
+    g = 5.0 / 3.0
+    rho, P, v, B = 2.0, 1.2, (0.5, -1.5, 0.25), (1.0, 0.0, 0.0)
+    n = (8, 4, 16)
+    p = inputs.uniform(n=n, gamma=g, rho=rho, P=P, v=v, B=B)
+    a2, ca2 = g * P / rho, B[0] ** 2 / rho
+    cf = [np.sqrt(max(a2, ca2)), np.sqrt(a2 + ca2), np.sqrt(a2 + ca2)]
+    expect = 0.4 * min((1.0 / n[a]) / (abs(v[a]) + cf[a]) for a in range(3))
+    assert make(p).compute_dt(0.4) == pytest.approx(expect, rel=1e-14)
+    # the minimum is taken over cells: one fast cell decides
+    st = {k: a.copy() for k, a in p.state.items()}
+    st["mz"][3, 2, 5] = rho * 7.0
+    st["E"][3, 2, 5] += 0.5 * rho * (7.0 ** 2 - v[2] ** 2)
+    o = orc.Oracle(*n, g, 1)
+    o.set_state(st)
+    assert o.compute_dt(0.3) == pytest.approx(0.3 * (1.0 / n[2]) / (7.0 + cf[2]), rel=1e-13)
+
+
+def wave_run(N, recon, wave="fast", axis=0, direction=1, nt=4):
+    n = [nt, nt, nt]
+    n[axis] = N
+    p = inputs.linear_wave(*n, wave=wave, axis=axis, direction=direction, recon=recon)
+    o = make(p)
+    run_to_time(o, p)
+    return inputs.wave_error(p.state, o.get_state())
+
+
+def test_T8_linear_wave_second_order_convergence():
+    # second-order convergence for PLM and PPM, PPM more accurate
+    e = {r: [wave_run(N, r) for N in (16, 32, 64)] for r in (1, 2)}
+    for r in (1, 2):
+        o1 = np.log2(e[r][0] / e[r][1])
+        o2 = np.log2(e[r][1] / e[r][2])
+        assert o2 > 1.9 and o1 > 1.4, (r, e[r])
+        assert e[r][2] < 2e-8
+    assert all(e[2][i] < e[1][i] for i in range(3))
+    # golden values: SURVEY.md 8(c) T8 "scratch" numbers, obtained there with an independent numpy
+    # implementation of the same readings (tests/golden/linear_wave_errors.txt)
+    gold = {}
+    for line in open(os.path.join(GOLD, "linear_wave_errors.txt")):
+        if line.strip() and not line.startswith("#"):
+            w, r, N, val = line.split()
+            gold[(w, int(r), int(N))] = float(val)
+    for r in (1, 2):
+        for i, N in enumerate((16, 32, 64)):
+            assert e[r][i] == pytest.approx(gold[("fast", r, N)], rel=2e-3)
+    assert wave_run(32, 1, "alfven") == pytest.approx(gold[("alfven", 1, 32)], rel=2e-3)
+    # slow wave (period 2, ~4x more steps): the survey's figure is reproduced to 0.7 %, inside its
+    # own stated "+- few %" band; the tight pins for this family are T9 and the convergence order
+    assert wave_run(32, 1, "slow") == pytest.approx(gold[("slow", 1, 32)], rel=1e-2)
+
+
+def test_T8b_amplitude_independent_error_is_truncation_not_bug():
+    # a linear scheme on a linear wave: the error scales with the amplitude
+    N = 16
+    errs = []
+    for A in (1e-6, 1e-7):
+        p = inputs.linear_wave(N, 4, 4, amplitude=A)
+        o = make(p)
+        run_to_time(o, p)
+        errs.append(inputs.wave_error(p.state, o.get_state()) / A)
+    assert errs[0] == pytest.approx(errs[1], rel=1e-3)
+
+
+def test_T9_sweeps_identical_along_axes_and_directions():
+    ref = wave_run(32, 1, axis=0)
+    for axis in (0, 1, 2):
+        for direction in (1, -1):
+            e = wave_run(32, 1, axis=axis, direction=direction)
+            assert e == pytest.approx(ref, rel=1e-9), (axis, direction)
+    refp = wave_run(16, 2, axis=0)
+    assert wave_run(16, 2, axis=1) == pytest.approx(refp, rel=1e-9)
+    assert wave_run(16, 2, axis=2, direction=-1) == pytest.approx(refp, rel=1e-9)
+
+
+@pytest.mark.parametrize("recon", [1, 2])
+def test_T10_divb_and_conservation(recon):
+    p = inputs.random_smooth(n=(16, 12, 10), seed=3, recon=recon)
+    o = make(p)
+    t0 = totals(p.state)
+    scale = {"rho": t0["rho"], "E": t0["E"], "mx": t0["rho"], "my": t0["rho"], "mz": t0["rho"]}
+    assert divb_normalised(p.state, p.n) < 1e-14
+    for s in range(5):
+        dt = o.compute_dt(p.cfl)
+        o.step(dt)
+        st = o.get_state()
+        assert divb_normalised(st, p.n) < 1e-14
+        t = totals(st)
+        for f in t:
+            assert abs(t[f] - t0[f]) / abs(scale[f]) < 5e-15 * (s + 1), (f, s)
+        # periodic images of the upper faces stay identical to the lower ones
+        assert np.array_equal(st["bx"][:, :, -1], st["bx"][:, :, 0])
+        assert np.array_equal(st["by"][:, -1, :], st["by"][:, 0, :])
+        assert np.array_equal(st["bz"][-1, :, :], st["bz"][0, :, :])
+    # the state really evolved
+    assert np.max(np.abs(st["rho"] - p.state["rho"])) > 1e-3
+    # face-averaged B (the magnetic flux through the box) is conserved too
+    for f in ("bx", "by", "bz"):
+        a0 = inputs._active(p.state[f], f).sum()
+        a1 = inputs._active(st[f], f).sum()
+        assert abs(a1 - a0) < 1e-12 * max(1.0, abs(a0))
+
+
+def test_half_step_is_first_order_update_with_half_dt():
+    # Step 5 (reading G8).  First-order fluxes do not depend on dt, so the
+    # half-state increment is exactly proportional to dt.
+    p = inputs.random_smooth(n=(8, 8, 8), seed=5)
+    incs = []
+    for dt in (1e-3, 2e-3):
+        o = make(p)
+        o.step(dt)
+        h = o.get_half_state()
+        incs.append({f: h[f] - p.state[f] for f in FIELDS})
+    for f in FIELDS:
+        np.testing.assert_allclose(incs[1][f], 2.0 * incs[0][f], rtol=0, atol=1e-14)
+    # and the factor is dt/2, not dt: hand-computed update of the two cells next to the single
+    # discontinuity of a planar x-only problem from point-wise HLLD fluxes
+    q = inputs.riemann("brio_wu", n_long=16, n_trans=2)
+    o = make(q)
+    dt = 1e-3
+    o.step(dt)
+    h = o.get_half_state()
+    g = q.gamma
+    st = q.state
+    # left and right primitive states of the single discontinuity between cells 7 and 8
+    WL = np.array([1.0, 0, 0, 0, 1.0, 1.0, 0.0])
+    WR = np.array([0.125, 0, 0, 0, 0.1, -1.0, 0.0])
+    Fd = orc.hlld(g, WL, WR, 0.75)
+    FL = orc.hlld(g, WL, WL, 0.75)
+    FR = orc.hlld(g, WR, WR, 0.75)
+    dx = 1.0 / 16
+    assert h["rho"][0, 0, 7] == pytest.approx(1.0 - 0.5 * dt / dx * (Fd[0] - FL[0]), abs=1e-15)
+    assert h["rho"][0, 0, 8] == pytest.approx(0.125 - 0.5 * dt / dx * (FR[0] - Fd[0]), abs=1e-15)
+    assert h["E"][0, 0, 7] == pytest.approx(st["E"][0, 0, 7] - 0.5 * dt / dx * (Fd[4] - FL[4]), abs=1e-14)
+    # B_y lives on y-faces at cell-centre x.  Eq. 21 with only E_z varying in x:
+    # B_y += (dt/2)/dx (E_z(i+1/2) - E_z(i-1/2)), and E_z on an x-face = -F[By-flux] (Table 1)
+    ez_d, ez_L = -Fd[5], -FL[5]
+    assert h["by"][0, 0, 7] == pytest.approx(1.0 + 0.5 * dt / dx * (ez_d - ez_L), abs=1e-15)
+
+
+def test_T12_brio_wu_planar_invariants_and_plateaus():
+    p = inputs.riemann("brio_wu", n_long=256, n_trans=4)
+    o = make(p)
+    n = run_to_time(o, p)
+    assert 200 < n < 300
+    st = o.get_state()
+    for f in FIELDS:
+        a = st[f]
+        ref = a[:1, :1, :]
+        assert np.array_equal(a, np.broadcast_to(ref, a.shape)), f   # all columns bit-identical
+    assert np.all(st["bx"] == 0.75)
+    assert np.max(np.abs(st["mz"])) <= 1e-15 and np.max(np.abs(st["bz"])) <= 1e-15
+    rho = st["rho"][0, 0]
+    by = 0.5 * (st["by"][0, 0] + st["by"][0, 1])
+    vx = st["mx"][0, 0] / rho
+    x = (np.arange(256) + 0.5) / 256
+    # SURVEY.md T12 plateau values (sanity, few-% level); standard Brio & Wu structure
+    sel = (x > 0.425) & (x < 0.455)
+    assert np.allclose(rho[sel], 0.676, atol=0.01)
+    sel = (x > 0.50) & (x < 0.53)
+    assert np.allclose(vx[sel], 0.600, atol=0.02) and np.allclose(by[sel], -0.534, atol=0.02)
+    assert np.allclose(rho[sel], 0.69, atol=0.02)
+    sel = (x > 0.58) & (x < 0.62)
+    assert np.allclose(rho[sel], 0.235, atol=0.01)
+    assert rho[-1] == 0.125 and rho[0] == 1.0
+    # no oscillations with PLM: total variation of rho close to the sum of jumps
+    tv = np.sum(np.abs(np.diff(rho)))
+    assert tv < 1.25          # sum of the monotone jumps is ~1.16
+    assert rho.min() > 0.1 and rho.max() <= 1.0 + 1e-12
+
+
+def test_T12b_riemann_identical_in_all_directions_and_orientations():
+    # identical results in all three directions and both orientations
+    base = None
+    for axis in (0, 1, 2):
+        for flip in (False, True):
+            p = inputs.riemann("brio_wu", n_long=64, n_trans=2, axis=axis, flip=flip)
+            o = make(p)
+            for _ in range(20):
+                o.step(o.compute_dt(0.4))
+            st = o.get_state()
+            rho = np.moveaxis(st["rho"], 2 - axis, -1)[0, 0]
+            if flip:
+                rho = rho[::-1]
+            if base is None:
+                base = rho
+            else:
+                np.testing.assert_allclose(rho, base, rtol=0, atol=2e-14)
+
+
+def test_T13_blast_symmetry_and_positivity():
+    # Point symmetry about the box centre (rho, E even; m odd; B even -- B is axial) and, with B
+    # along (1,1,1), invariance under the cyclic permutation x->y->z.  The scheme itself is
+    # symmetric to round-off on generic data (test_inversion_symmetry_generic_state).  On the blast
+    # the cell fields are symmetric to round-off after the first step, but the upwind switch of
+    # Eq. 16 ("v>0 / v<0 / otherwise") acts on mass fluxes that are zero up to
+    # round-off near the centre, and flips between mirror-image edges; the difference between its
+    # branches is a truncation-level quantity, so a handful of faces differ at ~1e-3 at once and
+    # the asymmetry then spreads at ~1e-4..1e-2 of the blast amplitude.
+    # That is a property of the published algorithm, not pinned here
+    # beyond a loose bound.
+    inv = lambda a: a[::-1, ::-1, ::-1]
+    for recon in (1, 2):
+        p = inputs.blast(n=24, n_steps=12, recon=recon)
+        o = make(p)
+        o.step(o.compute_dt(p.cfl))
+        st = o.get_state()
+        assert np.max(np.abs(st["rho"] - inv(st["rho"]))) < 1e-14
+        assert np.max(np.abs(st["E"] - inv(st["E"]))) < 1e-13
+        for f in ("mx", "my", "mz"):
+            assert np.max(np.abs(st[f] + inv(st[f]))) < 1e-14
+        # B: symmetric except on the few faces next to edges whose mass flux is zero up to
+        # round-off (24 of 14400 per component at n=24) -- the Eq. 16 switch, see above
+        for f in ("bx", "by", "bz"):
+            bad = np.abs(st[f] - inv(st[f])) > 1e-13
+            assert bad.sum() <= 0.005 * bad.size, (recon, f, int(bad.sum()))
+        assert np.max(np.abs(st["rho"] - np.transpose(st["rho"], (1, 2, 0)))) < 1e-14
+        assert np.max(np.abs(st["mx"] - np.transpose(st["mz"], (1, 2, 0)))) < 1e-14
+        run_steps(o, p, p.n_steps - 1)
+        st = o.get_state()
+        g = p.gamma
+        rho = st["rho"]
+        bcx, bcy, bcz = inputs.cell_centred_b(st)
+        v2 = (st["mx"] ** 2 + st["my"] ** 2 + st["mz"] ** 2) / rho ** 2
+        P = (g - 1) * (st["E"] - 0.5 * rho * v2 - 0.5 * (bcx ** 2 + bcy ** 2 + bcz ** 2))
+        assert np.all(np.isfinite(rho)) and rho.min() > 0.02 and P.min() > 0.02
+        amp = np.max(np.abs(rho - 1.0))
+        assert amp > 0.3                                  # the blast did something
+        assert np.max(np.abs(rho - inv(rho))) < 0.05 * amp
+        assert divb_normalised(st, p.n) < 1e-13
+
+
+def test_inversion_symmetry_generic_state():
+    # rho(x) -> rho(-x), m -> -m(-x), B -> B(-x) commutes with one step to round-off
+    inv = lambda a: np.ascontiguousarray(a[::-1, ::-1, ::-1])
+
+    def invert(st):
+        out = {f: inv(st[f]) for f in st}
+        for f in ("mx", "my", "mz"):
+            out[f] = -out[f]
+        return out
+    for recon in (1, 2):
+        p = inputs.random_smooth(n=(12, 10, 8), seed=2, recon=recon)
+        o = make(p)
+        dt = o.compute_dt(0.4)
+        o.step(dt)
+        a = o.get_state()
+        o.set_state(invert(p.state))
+        o.step(dt)
+        b = invert(o.get_state())
+        for f in FIELDS:
+            assert np.max(np.abs(a[f] - b[f])) < 5e-15, (recon, f)
+
+
+# ----------------------------------------------------------------------------- T14 hydro limit
+def sod_exact(x, t, gamma=1.4):
+    """Exact solution of the Sod problem (rho,u,p)_L=(1,0,1), (0.125,0,0.1), textbook (Toro ch. 4)."""
+    rl, pl, rr, pr = 1.0, 1.0, 0.125, 0.1
+    al, ar = np.sqrt(gamma * pl / rl), np.sqrt(gamma * pr / rr)
+    g1, g2 = (gamma - 1) / (2 * gamma), (gamma + 1) / (2 * gamma)
+
+    def f(p):   # pressure function: left rarefaction + right shock
+        fl = 2 * al / (gamma - 1) * ((p / pl) ** g1 - 1)
+        A, B = 2 / ((gamma + 1) * rr), (gamma - 1) / (gamma + 1) * pr
+        fr = (p - pr) * np.sqrt(A / (p + B))
+        return fl + fr
+    lo, hi = 1e-6, 1.0
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        if f(mid) > 0:
+            hi = mid
+        else:
+            lo = mid
+    ps = 0.5 * (lo + hi)
+    us = 2 * al / (gamma - 1) * (1 - (ps / pl) ** g1)
+    rsl = rl * (ps / pl) ** (1 / gamma)
+    rsr = rr * ((ps / pr + (gamma - 1) / (gamma + 1)) / ((gamma - 1) / (gamma + 1) * ps / pr + 1))
+    S = ar * np.sqrt(g2 * ps / pr + g1)
+    asl = al * (ps / pl) ** g1
+    xi = (x - 0.5) / t
+    rho = np.where(xi < -al, rl, np.where(xi < us - asl,
+          rl * (2 / (gamma + 1) + (gamma - 1) / ((gamma + 1) * al) * (-xi)) ** (2 / (gamma - 1)),
+          np.where(xi < us, rsl, np.where(xi < S, rsr, rr))))
+    return rho
+
+
+def test_T14_hydro_limit_sod_converges_to_exact_solution():
+    errs = []
+    for N in (64, 128, 256):
+        g = 1.4
+        x = (np.arange(N) + 0.5) / N
+        left = x < 0.5
+        one = np.ones((2, 2, N))
+        rho = np.where(left, 1.0, 0.125) * one
+        P = np.where(left, 1.0, 0.1) * one
+        sh = inputs.field_shapes(N, 2, 2)
+        st = inputs.from_primitives(rho, 0 * one, 0 * one, 0 * one, P, np.zeros(sh["bx"]),
+                                    np.zeros(sh["by"]), np.zeros(sh["bz"]), g)
+        p = inputs.Problem("sod", (N, 2, 2), g, st, bc=(1, 0, 0), recon=1, t_end=0.2)
+        o = make(p)
+        run_to_time(o, p)
+        out = o.get_state()
+        assert np.all(out["bx"] == 0) and np.all(out["by"] == 0) and np.all(out["bz"] == 0)
+        errs.append(np.mean(np.abs(out["rho"][0, 0] - sod_exact(x, 0.2, g))))
+    assert errs[0] < 0.012 and errs[2] < 0.004
+    assert errs[0] / errs[1] > 1.6 and errs[1] / errs[2] > 1.6     # ~1st order at discontinuities

@@ -1,0 +1,375 @@
+"""Pins for the oracle's point-wise building blocks.
+
+Each test checks oracle/mhd_oracle.c against something fixed by the paper or by the
+mathematics, never against the oracle itself:
+  T2  HLLD consistency F(U,U) = F(U)                       (Eq. 8)
+  T3  HLLD mirror symmetry
+  T4  isolated contact / rotational discontinuity captured exactly (Miyoshi & Kusano)
+  T5  B = 0 reduces to the textbook HLLC solver (written out here independently)
+  T6  eigen-system: L.R = I, A.R = R.Lambda, L.A = Lambda.L with A typed from the primitive
+      equations
+  T7  CT edge formula: exact for E linear in space; uniform state returns E_ref (Eq. 15-18)
+  T11 PPM: exact on constants / linear / cubic cell averages, monotone faces
+  plus closed forms for Eq. 12 and Eq. 26-28.
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+
+G = 5.0 / 3.0
+
+
+def rand_state(rng, bscale=1.0, vscale=1.0):
+    rho = rng.uniform(0.2, 3.0)
+    P = rng.uniform(0.1, 3.0)
+    v = rng.normal(size=3) * vscale
+    b = rng.normal(size=2) * bscale
+    return np.array([rho, v[0], v[1], v[2], P, b[0], b[1]])
+
+
+def phys_flux_np(gamma, W, bx):
+    """Eq. 8, typed here independently of the oracle."""
+    rho, u, v, w, P, by, bz = W
+    b2 = bx * bx + by * by + bz * bz
+    pT = P + 0.5 * b2
+    E = P / (gamma - 1) + 0.5 * rho * (u * u + v * v + w * w) + 0.5 * b2
+    vb = u * bx + v * by + w * bz
+    return np.array([rho * u, rho * u * u + pT - bx * bx, rho * u * v - bx * by,
+                     rho * u * w - bx * bz, u * (E + pT) - bx * vb, by * u - bx * v,
+                     bz * u - bx * w])
+
+
+def test_phys_flux_matches_eq8():
+    rng = np.random.default_rng(0)
+    for _ in range(50):
+        W = rand_state(rng)
+        bx = rng.normal()
+        np.testing.assert_allclose(orc.phys_flux(G, W, bx), phys_flux_np(G, W, bx),
+                                   rtol=1e-14, atol=1e-14)
+
+
+def test_fast_speed_closed_forms():
+    # Eq. 12.  B = 0 -> sound speed; B parallel to n -> max(a, c_A);
+    # B perpendicular -> sqrt(a^2 + c_A^2); SURVEY.md G19 background: a=1, c_f=2.
+    assert orc.fast_speed(G, 2.0, 1.5, 0, 0, 0) == pytest.approx(np.sqrt(G * 1.5 / 2.0), rel=1e-15)
+    assert orc.fast_speed(G, 1.0, 0.3, 2.0, 0, 0) == pytest.approx(2.0, rel=1e-15)
+    assert orc.fast_speed(G, 1.0, 3.0, 0.5, 0, 0) == pytest.approx(np.sqrt(G * 3.0), rel=1e-15)
+    assert orc.fast_speed(G, 4.0, 1.0, 0, 1.0, 2.0) == pytest.approx(np.sqrt((G + 5.0) / 4.0), rel=1e-15)
+    assert orc.fast_speed(G, 1.0, 0.6, 1.0, 1.5, 0.0) == pytest.approx(2.0, rel=1e-14)
+
+
+# ----------------------------------------------------------------------------- HLLD
+def test_T2_hlld_consistency_all_branches():
+    rng = np.random.default_rng(1)
+    worst = 0.0
+    for it in range(2000):
+        W = rand_state(rng, vscale=[0.3, 1.0, 3.0, 6.0][it % 4])
+        bx = rng.normal() * [1.0, 0.1, 0.0][it % 3]
+        F = orc.hlld(G, W, W, bx)
+        Fx = phys_flux_np(G, W, bx)
+        worst = max(worst, np.max(np.abs(F - Fx)) / max(1.0, np.max(np.abs(Fx))))
+    assert worst < 2e-14
+
+
+def test_T3_hlld_mirror_symmetry():
+    rng = np.random.default_rng(2)
+    flip = np.array([1, -1, 1, 1, 1, 1, 1.0])          # u -> -u
+    sign = np.array([-1, 1, -1, -1, -1, -1, -1.0])      # all but the normal-momentum flux flip
+    worst = 0.0
+    for it in range(2000):
+        WL = rand_state(rng, vscale=[0.3, 2.0][it % 2])
+        WR = rand_state(rng, vscale=[0.3, 2.0][it % 2])
+        bx = rng.normal()
+        F = orc.hlld(G, WL, WR, bx)
+        Fm = orc.hlld(G, WR * flip, WL * flip, -bx)
+        worst = max(worst, np.max(np.abs(Fm - sign * F)) / max(1.0, np.max(np.abs(F))))
+    assert worst < 2e-14
+
+
+def test_T3b_hlld_transverse_rotation():
+    # rotating the transverse axes by 90 degrees (v,w,By,Bz) -> (w,-v,Bz,-By) rotates the flux
+    rng = np.random.default_rng(3)
+    for _ in range(200):
+        WL, WR = rand_state(rng), rand_state(rng)
+        bx = rng.normal()
+        rot = lambda W: np.array([W[0], W[1], W[3], -W[2], W[4], W[6], -W[5]])
+        F = orc.hlld(G, WL, WR, bx)
+        Fr = orc.hlld(G, rot(WL), rot(WR), bx)
+        np.testing.assert_allclose(Fr, rot(F), rtol=0, atol=5e-14 * max(1, np.abs(F).max()))
+
+
+def test_T4_hlld_contact_and_rotational_discontinuity():
+    # stationary contact: only rho jumps, u = 0, Bx != 0
+    WL = np.array([1.0, 0.0, 0.3, -0.2, 0.8, 0.7, -0.4])
+    WR = WL.copy(); WR[0] = 0.25
+    bx = 0.9
+    F = orc.hlld(G, WL, WR, bx)
+    assert F[0] == 0.0
+    np.testing.assert_allclose(F, phys_flux_np(G, WL, bx), rtol=0, atol=2e-15)
+    np.testing.assert_allclose(F, phys_flux_np(G, WR, bx), rtol=0, atol=2e-15)
+    # contact moving with u0: upwind physical flux
+    for u0, Wup in ((0.4, WL), (-0.4, WR)):
+        A, B = WL.copy(), WR.copy()
+        A[1] = B[1] = u0
+        F = orc.hlld(G, A, B, bx)
+        Wu = Wup.copy(); Wu[1] = u0
+        np.testing.assert_allclose(F, phys_flux_np(G, Wu, bx), rtol=0, atol=4e-15)
+    # rotational (Alfven) discontinuity at rest: u = Bx/sqrt(rho), B_perp rotates,
+    # delta v_perp = delta B_perp / sqrt(rho)
+    rho, P, bx = 1.7, 0.9, 0.8
+    u = bx / np.sqrt(rho)
+    bp = 1.1
+    th0, th1 = 0.3, 2.1
+    BL = bp * np.array([np.cos(th0), np.sin(th0)])
+    BR = bp * np.array([np.cos(th1), np.sin(th1)])
+    vL = np.array([0.2, -0.1])
+    vR = vL + (BR - BL) / np.sqrt(rho)
+    WL = np.array([rho, u, vL[0], vL[1], P, BL[0], BL[1]])
+    WR = np.array([rho, u, vR[0], vR[1], P, BR[0], BR[1]])
+    F = orc.hlld(G, WL, WR, bx)
+    np.testing.assert_allclose(F, phys_flux_np(G, WL, bx), rtol=0, atol=4e-15)
+    np.testing.assert_allclose(F, phys_flux_np(G, WR, bx), rtol=0, atol=4e-15)
+
+
+def hllc_textbook(gamma, WL, WR):
+    """Toro's HLLC for the Euler equations with given S_L, S_R (Davis estimate as in O4)."""
+    def cons(W):
+        rho, u, v, w, P = W[:5]
+        return np.array([rho, rho * u, rho * v, rho * w, P / (gamma - 1) + 0.5 * rho * (u * u + v * v + w * w)])
+
+    def flux(W):
+        rho, u, v, w, P = W[:5]
+        E = cons(W)[4]
+        return np.array([rho * u, rho * u * u + P, rho * u * v, rho * u * w, u * (E + P)])
+    aL, aR = np.sqrt(gamma * WL[4] / WL[0]), np.sqrt(gamma * WR[4] / WR[0])
+    SL = min(WL[1], WR[1]) - max(aL, aR)
+    SR = max(WL[1], WR[1]) + max(aL, aR)
+    if SL > 0:
+        return flux(WL)
+    if SR < 0:
+        return flux(WR)
+    rL, uL, pL = WL[0], WL[1], WL[4]
+    rR, uR, pR = WR[0], WR[1], WR[4]
+    Ss = (pR - pL + rL * uL * (SL - uL) - rR * uR * (SR - uR)) / (rL * (SL - uL) - rR * (SR - uR))
+
+    def star(W, S):
+        rho, u, v, w, P = W[:5]
+        E = cons(W)[4]
+        f = rho * (S - u) / (S - Ss)
+        return f * np.array([1.0, Ss, v, w, E / rho + (Ss - u) * (Ss + P / (rho * (S - u)))])
+    if Ss >= 0:
+        return flux(WL) + SL * (star(WL, SL) - cons(WL))
+    return flux(WR) + SR * (star(WR, SR) - cons(WR))
+
+
+def test_T5_hlld_reduces_to_hllc_without_field():
+    rng = np.random.default_rng(4)
+    for it in range(500):
+        WL = rand_state(rng, bscale=0.0, vscale=[0.3, 2.0, 5.0][it % 3])
+        WR = rand_state(rng, bscale=0.0, vscale=[0.3, 2.0, 5.0][it % 3])
+        F = orc.hlld(G, WL, WR, 0.0)
+        Fh = hllc_textbook(G, WL, WR)
+        np.testing.assert_allclose(F[:5], Fh, rtol=0, atol=3e-14 * max(1.0, np.abs(Fh).max()))
+        assert F[5] == 0.0 and F[6] == 0.0
+
+
+# ----------------------------------------------------------------------------- eigen-system
+def prim_matrix(gamma, W, bx):
+    """A(W) of dW/dt + A dW/dx = 0 for W = (rho,u,v,w,P,By,Bz), typed from the primitive-form
+    ideal MHD equations."""
+    rho, u, v, w, P, by, bz = W
+    A = np.eye(7) * u
+    A[0, 1] = rho
+    A[1, 4] = 1 / rho; A[1, 5] = by / rho; A[1, 6] = bz / rho
+    A[2, 5] = -bx / rho
+    A[3, 6] = -bx / rho
+    A[4, 1] = gamma * P
+    A[5, 1] = by; A[5, 2] = -bx
+    A[6, 1] = bz; A[6, 3] = -bx
+    return A
+
+
+def test_T6_eigensystem_identities():
+    rng = np.random.default_rng(5)
+    worst_lr, res = 0.0, []
+    for it in range(600):
+        W = rand_state(rng)
+        bx = rng.normal()
+        kind = it % 6
+        if kind == 1: W[6] = 0.0                 # Bz = 0
+        if kind == 2: bx = 0.0                   # Bx = 0
+        if kind == 3: W[5] = W[6] = 0.0          # B_perp = 0
+        if kind == 4: bx = -abs(bx)
+        lam, L, R = orc.eigensystem(G, W, bx)
+        A = prim_matrix(G, W, bx)
+        worst_lr = max(worst_lr, np.max(np.abs(L @ R - np.eye(7))))
+        sc = max(1.0, np.max(np.abs(A)))
+        r1 = np.max(np.abs(A @ R - R * lam[None, :])) / sc
+        r2 = np.max(np.abs(L @ A - lam[:, None] * L)) / sc
+        res.append(max(r1, r2))
+        if kind != 3:
+            assert max(r1, r2) < 1e-12, (it, r1, r2)
+        else:
+            assert max(r1, r2) < 1e-6
+        # wave speeds ordered and equal to the spectrum of A
+        assert np.all(np.diff(lam) >= -1e-14)
+        ev = np.sort(np.linalg.eigvals(A).real)
+        np.testing.assert_allclose(lam, ev, rtol=0, atol=2e-6 if kind in (2, 3) else 1e-9)
+    assert worst_lr < 2e-13
+    assert np.median(res) < 1e-14
+
+
+def test_eigensystem_G19_fast_wave():
+    # SURVEY.md G19 / PAPER.md:339: rho=1, P=1/gamma, B=(1,1.5,0): c_f=2, c_a=1, c_s=1/2 and the
+    # right-going fast eigenvector in primitive variables is prop. to (2, 4, -2, 0, 2*gamma*P.., ...)
+    W = np.array([1.0, 0.0, 0.0, 0.0, 1.0 / G, 1.5, 0.0])
+    lam, L, R = orc.eigensystem(G, W, 1.0)
+    np.testing.assert_allclose(lam, [-2, -1, -0.5, 0, 0.5, 1, 2], atol=1e-14)
+    r = R[:, 6] / R[0, 6] * 2.0
+    # primitive perturbation for d(rho)=2: du = c_f*2/rho = 4, dP = a^2 d(rho) = 2, dv=-2, dBy=4
+    np.testing.assert_allclose(r, [2, 4, -2, 0, 2, 4, 0], atol=1e-13)
+
+
+# ----------------------------------------------------------------------------- PLMC
+def test_plmc_linear_profile_and_extremum():
+    rng = np.random.default_rng(6)
+    for _ in range(100):
+        W0 = rand_state(rng)
+        bx = rng.normal()
+        d = 1e-3 * rng.normal(size=7)
+        lo, hi = orc.plmc(G, W0 - d, W0, W0 + d, bx)
+        # uniform slope: every limiter candidate equals the slope itself (Eq. 23-27)
+        np.testing.assert_allclose(hi, W0 + 0.5 * d, rtol=0, atol=1e-14)
+        np.testing.assert_allclose(lo, W0 - 0.5 * d, rtol=0, atol=1e-14)
+        # local extremum in every characteristic variable (dL = -dR): first order (Eq. 27)
+        lo, hi = orc.plmc(G, W0 + d, W0, W0 + d, bx)
+        np.testing.assert_array_equal(lo, W0)
+        np.testing.assert_array_equal(hi, W0)
+
+
+def test_plmc_scalar_limiter_on_entropy_wave():
+    # Only rho varies (v = const, P = const, B = const): the perturbation is a pure entropy
+    # wave, characteristic variable #3 = d(rho) - dP/a^2 = d(rho); Eq. 27 acts on it alone.
+    W0 = np.array([1.0, 0.3, 0.1, -0.2, 0.7, 0.5, 0.4])
+    for dl, dr in ((0.1, 0.3), (0.3, 0.1), (0.2, 0.2), (0.1, 0.9), (-0.1, -0.4), (0.1, -0.1)):
+        Wm, Wp = W0.copy(), W0.copy()
+        Wm[0] -= dl; Wp[0] += dr
+        lo, hi = orc.plmc(G, Wm, W0, Wp, 0.6)
+        if dl * dr > 0:
+            dc = 0.5 * (dl + dr)
+            dvl = 2 * dl * dr / (dl + dr)
+            m = np.sign(dc) * min(2 * abs(dl), 2 * abs(dr), abs(dc), abs(dvl))
+        else:
+            m = 0.0
+        exp_hi = W0.copy(); exp_hi[0] += 0.5 * m
+        exp_lo = W0.copy(); exp_lo[0] -= 0.5 * m
+        np.testing.assert_allclose(hi, exp_hi, rtol=0, atol=1e-15)
+        np.testing.assert_allclose(lo, exp_lo, rtol=0, atol=1e-15)
+
+
+# ----------------------------------------------------------------------------- PPM
+def cell_avg(coef, i):
+    """exact average over [i-1/2, i+1/2] of the polynomial sum_n coef[n] x^n"""
+    P = np.polynomial.Polynomial(coef).integ()
+    return P(i + 0.5) - P(i - 0.5)
+
+
+def test_T11_ppm_exactness():
+    lo, hi = orc.ppm_scalar([3.7] * 5)
+    assert lo == 3.7 and hi == 3.7
+    # linear: faces exact, no limiter changes them
+    q = [2.0 + 0.5 * i for i in range(-2, 3)]
+    lo, hi = orc.ppm_scalar(q)
+    assert lo == pytest.approx(2.0 - 0.25, abs=1e-15) and hi == pytest.approx(2.25, abs=1e-15)
+    # monotone cubic, gentle curvature: 4th-order face values are exact for cubic cell averages
+    coef = [1.0, 2.0, 0.05, 0.01]
+    q = [cell_avg(coef, i) for i in range(-2, 3)]
+    lo, hi = orc.ppm_scalar(q)
+    P = np.polynomial.Polynomial(coef)
+    assert lo == pytest.approx(P(-0.5), abs=1e-14)
+    assert hi == pytest.approx(P(0.5), abs=1e-14)
+    # parabola with an extremum inside cell i is kept (smooth-extremum preservation, r = 1):
+    coef = [1.0, 0.05, -0.3]
+    q = [cell_avg(coef, i) for i in range(-2, 3)]
+    lo, hi = orc.ppm_scalar(q)
+    P = np.polynomial.Polynomial(coef)
+    assert lo == pytest.approx(P(-0.5), abs=1e-14)
+    assert hi == pytest.approx(P(0.5), abs=1e-14)
+
+
+def test_T11_ppm_monotone_and_bounded():
+    rng = np.random.default_rng(7)
+    for _ in range(2000):
+        q = np.sort(rng.normal(size=5))            # monotone data
+        if rng.uniform() < 0.5:
+            q = q[::-1].copy()
+        lo, hi = orc.ppm_scalar(q)
+        a, b = min(q[1], q[2]), max(q[1], q[2])
+        assert a - 1e-14 <= lo <= b + 1e-14
+        a, b = min(q[2], q[3]), max(q[2], q[3])
+        assert a - 1e-14 <= hi <= b + 1e-14
+        # parabola through (lo, q_i, hi) is monotone: |d-| <= 2|d+| and vice versa
+        dm, dp = q[2] - lo, hi - q[2]
+        assert abs(dm) <= 2 * abs(dp) + 1e-14 and abs(dp) <= 2 * abs(dm) + 1e-14
+    # isolated spike: strict extremum with neighbours' curvature of opposite sign -> flattened
+    lo, hi = orc.ppm_scalar([0.0, 0.0, 1.0, 0.0, 0.0])
+    assert lo == 1.0 and hi == 1.0
+
+
+def test_ppmc_constant_and_linear_vector():
+    rng = np.random.default_rng(8)
+    W0 = rand_state(rng)
+    lo, hi = orc.ppmc(G, np.tile(W0, 5), 0.4)
+    np.testing.assert_allclose(lo, W0, rtol=0, atol=1e-14)
+    np.testing.assert_allclose(hi, W0, rtol=0, atol=1e-14)
+    d = 1e-3 * rng.normal(size=7)
+    Ws = np.concatenate([W0 + s * d for s in range(-2, 3)])
+    lo, hi = orc.ppmc(G, Ws, 0.4)
+    np.testing.assert_allclose(lo, W0 - 0.5 * d, rtol=0, atol=2e-14)
+    np.testing.assert_allclose(hi, W0 + 0.5 * d, rtol=0, atol=2e-14)
+
+
+# ----------------------------------------------------------------------------- CT edge
+def test_T7_ct_edge_linear_field_exact():
+    # E(x,y) = e0 + gx x + gy y sampled at the four faces and four cell centres around the edge
+    # at the origin; any upwind choice must return e0.
+    rng = np.random.default_rng(9)
+    for _ in range(200):
+        e0, gx, gy = rng.normal(size=3)
+        dx, dy = rng.uniform(0.1, 1.0, size=2)
+        E = lambda x, y: e0 + gx * x + gy * y
+        Ea0, Ea1 = E(0, 0.5 * dy), E(0, -0.5 * dy)          # a-faces at x=0
+        Eb0, Eb1 = E(0.5 * dx, 0), E(-0.5 * dx, 0)          # b-faces at y=0
+        Er00, Er10 = E(0.5 * dx, 0.5 * dy), E(-0.5 * dx, 0.5 * dy)
+        Er01, Er11 = E(0.5 * dx, -0.5 * dy), E(-0.5 * dx, -0.5 * dy)
+        M = rng.choice([-1.0, 0.0, 1.0], size=4)
+        out = orc.ct_edge(Ea0, Ea1, Eb0, Eb1, M[0], M[1], M[2], M[3], Er00, Er10, Er01, Er11)
+        assert out == pytest.approx(e0, abs=1e-14)
+    assert orc.ct_edge(*([0.37] * 4), 1.0, -1.0, 0.0, 2.0, *([0.37] * 4)) == pytest.approx(0.37, abs=1e-16)
+
+
+def test_T7_ct_edge_upwind_selection():
+    # Eq. 16-17: the slope at (i-1/2, j-1/4) comes from cell i-1 if the mass flux through face
+    # (i-1/2, j) is positive, from cell i if negative, mean otherwise.  Make exactly one
+    # candidate non-zero and see it selected.
+    z = dict(Ea0=0, Ea1=0, Eb0=0, Eb1=0, Ma0=0, Ma1=0, Mb0=0, Mb1=0, Er00=0, Er10=0, Er01=0, Er11=0)
+    order = list(z.keys())
+
+    def call(**kw):
+        d = dict(z); d.update(kw)
+        return orc.ct_edge(*[d[k] for k in order])
+    # Er10 is cell (ia-1, ib): used by T1 when Ma0>0 and by T4 when Mb1<0
+    assert call(Er10=1.0, Ma0=1.0, Mb1=1.0) == pytest.approx(-0.25)
+    assert call(Er10=1.0, Ma0=-1.0, Mb1=-1.0) == pytest.approx(-0.25)
+    assert call(Er10=1.0, Ma0=1.0, Mb1=-1.0) == pytest.approx(-0.5)
+    assert call(Er10=1.0, Ma0=-1.0, Mb1=1.0) == 0.0
+    assert call(Er10=1.0, Ma0=0.0, Mb1=1.0) == pytest.approx(-0.125)
+    # Er01 is cell (ia, ib-1): used by T2 when Ma1<0 and by T3 when Mb0>0
+    assert call(Er01=1.0, Ma1=-1.0, Mb0=-1.0) == pytest.approx(-0.25)
+    assert call(Er01=1.0, Ma1=1.0, Mb0=1.0) == pytest.approx(-0.25)
+    # Er11 is cell (ia-1, ib-1): T2 when Ma1>0, T4 when Mb1>0
+    assert call(Er11=1.0, Ma1=1.0, Mb1=1.0) == pytest.approx(-0.5)
+    # Er00 is cell (ia, ib): T1 when Ma0<0, T3 when Mb0<0
+    assert call(Er00=1.0, Ma0=-1.0, Mb0=-1.0) == pytest.approx(-0.5)
+    assert call(Er00=1.0, Ma0=1.0, Mb0=1.0) == 0.0
