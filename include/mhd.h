@@ -1,0 +1,131 @@
+/*
+ * include/mhd.h -- C ABI of libmhd.so: the fp64 Van Leer + Constrained Transport (VL+CT)
+ * ideal-MHD time step of Cholla-MHD (arxiv 2402.05240) as hand-written CUDA for sm_100a.
+ *
+ * Citations are to /root/reference/PAPER.md (line numbers) and to the readings O0..O12 /
+ * G1..G24 restated in DESIGN.md.
+ *
+ * Conventions
+ *   - One global context per process (one GPU, no MPI: BASELINE.json north_star).
+ *   - Unit box, Delta_a = 1/n_a.  Cells (i,j,k), i fastest.
+ *   - State = 8 fp64 SoA fields: rho, mx, my, mz, E at cell centres,
+ *     nx*ny*nz values each, index i + nx*(j + ny*k);  bx on x-faces, (nx+1)*ny*nz values,
+ *     index i + (nx+1)*(j + ny*k); by nx*(ny+1)*nz; bz nx*ny*(nz+1).  Face index f is the
+ *     LOWER face of cell f (position f-1/2; Eq. 20 indexing B_{x,i-1/2}).
+ *   - "host" pointers are ordinary CPU memory (pageable or pinned), "device" pointers are
+ *     CUDA device memory of the current device.  The caller owns every buffer it passes;
+ *     the library owns its internal device arrays (or the workspace handed to
+ *     mhd_init_workspace, which the caller must keep alive until mhd_finalize).
+ *   - All kernels are launched on the library's stream (default: the legacy default stream;
+ *     change with mhd_set_stream).  Calls are asynchronous on that stream unless stated.
+ *   - Every function returns MHD_OK (0) or a negative MHD_ERR_* code; nothing throws or
+ *     aborts across the ABI.  mhd_last_error() gives a static human-readable string.
+ *   - No floors or fix-ups are applied to the state (the paper describes none, G18).  A
+ *     non-physical state (rho <= 0, P <= 0 or non-finite) seen by the CFL kernel makes
+ *     mhd_compute_dt return MHD_ERR_UNPHYSICAL.
+ */
+#ifndef MHD_H_
+#define MHD_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MHD_OK 0
+#define MHD_ERR_ARG (-1)        /* bad argument */
+#define MHD_ERR_NOT_INIT (-2)   /* mhd_init has not been called */
+#define MHD_ERR_NOMEM (-3)      /* device allocation failed / workspace too small */
+#define MHD_ERR_CUDA (-4)       /* a CUDA call failed; see mhd_last_error() */
+#define MHD_ERR_UNPHYSICAL (-5) /* rho <= 0, P <= 0 or non-finite value in the state */
+
+#define MHD_RECON_PCM 0  /* Eq. 14, PAPER.md:139-147 (debug: first order everywhere) */
+#define MHD_RECON_PLMC 1 /* Eq. 23-28 */
+#define MHD_RECON_PPMC 2 /* PAPER.md:231, 431; reading O10 */
+
+#define MHD_BC_PERIODIC 0
+#define MHD_BC_OUTFLOW 1 /* zero-gradient copy of the nearest active cell/face (O12) */
+
+/* Number of bytes of device memory the context for an nx*ny*nz grid with this
+ * reconstruction needs (state, half-step state, face fluxes, edge fields, scratch).
+ * Returns 0 on bad arguments. */
+size_t mhd_workspace_bytes(int nx, int ny, int nz, int recon);
+
+/* Create the context (the nine-step VL+CT list): nx*ny*nz cells on the unit
+ * box, adiabatic index gamma > 1, recon one of MHD_RECON_*.  All axes periodic
+ * until mhd_set_boundary says otherwise.  Device memory is obtained with cudaMalloc.
+ * A previous context is destroyed first. */
+int mhd_init(int nx, int ny, int nz, double gamma, int recon);
+
+/* Same, but all device arrays are carved out of `workspace` (a DEVICE pointer, 256-byte
+ * aligned, at least mhd_workspace_bytes() long, e.g. a torch tensor's data_ptr()).  The
+ * library never frees it. */
+int mhd_init_workspace(int nx, int ny, int nz, double gamma, int recon, void *workspace,
+                       size_t workspace_bytes);
+
+/* axis 0/1/2 = x/y/z; kind MHD_BC_*.  Takes effect at the next ghost fill (the next
+ * mhd_set_state* or mhd_step). */
+int mhd_set_boundary(int axis, int kind);
+
+/* cudaStream_t (as void*) on which all later work is launched; NULL = default stream. */
+int mhd_set_stream(void *cuda_stream);
+
+/* Copy a full state in from 8 HOST arrays (layout above) and fill the ghost layers.
+ * Synchronous with respect to the host buffers (they may be reused on return). */
+int mhd_set_state(const double *rho, const double *mx, const double *my, const double *mz,
+                  const double *E, const double *bx, const double *by, const double *bz);
+
+/* Same with 8 DEVICE arrays; asynchronous on the library stream. */
+int mhd_set_state_device(const double *rho, const double *mx, const double *my,
+                         const double *mz, const double *E, const double *bx,
+                         const double *by, const double *bz);
+
+/* Eq. 11-12: dt = cfl * min over cells and directions of
+ * Delta_a / (|v_a| + c_f,a), by a warp-shuffle + block + atomic-min reduction
+ * (PAPER.md:317-327).  Synchronous: *dt (HOST pointer) is valid on return. */
+int mhd_compute_dt(double cfl, double *dt);
+
+/* One full VL+CT step of size dt (steps 2-9): ghost fill, PCM+HLLD
+ * predictor fluxes, CT edge fields, half update, high-order reconstruction + HLLD, CT edge
+ * fields, full update.  Asynchronous on the library stream. */
+int mhd_step(double dt);
+
+/* n_steps times { dt = cfl * CFL minimum on the device; full step with that dt } without
+ * any host synchronisation; the dt of each step stays on the device.  If t_accum is
+ * non-NULL (HOST pointer) the call synchronises and stores the sum of the dt taken. */
+int mhd_advance(int n_steps, double cfl, double *t_accum);
+
+/* Copy the state out to 8 HOST arrays (any pointer may be NULL = skip).  Synchronises. */
+int mhd_get_state(double *rho, double *mx, double *my, double *mz, double *E, double *bx,
+                  double *by, double *bz);
+
+/* Same to 8 DEVICE arrays; asynchronous on the library stream. */
+int mhd_get_state_device(double *rho, double *mx, double *my, double *mz, double *E,
+                         double *bx, double *by, double *bz);
+
+/* Debug/parity: the predictor's U^{n+1/2} left by the last mhd_step,
+ * to HOST arrays.  Synchronises. */
+int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *E, double *bx,
+                       double *by, double *bz);
+
+/* max over active cells of |sum_a (B_a[upper] - B_a[lower]) / Delta_a|.
+ * Synchronous; *out is a HOST pointer. */
+int mhd_max_divb(double *out);
+
+/* Number of kernel launches issued by this library since mhd_init (for bench.py). */
+long long mhd_launch_count(void);
+
+/* Block until all work on the library stream is done. */
+int mhd_synchronize(void);
+
+/* Free everything.  Safe to call twice. */
+int mhd_finalize(void);
+
+/* Static string describing the last error (never NULL). */
+const char *mhd_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MHD_H_ */

@@ -1,0 +1,429 @@
+// mhd_api.cu -- C ABI (include/mhd.h) of the B200 VL+CT ideal-MHD step: context, memory
+// carving, launch sequence of one step.  Pure CUDA runtime; no torch types.
+#include <cstdio>
+#include <cstring>
+#include <cuda_runtime.h>
+
+#include "../../include/mhd.h"
+#include "mhd_kernels.cuh"
+
+using namespace mhd;
+
+namespace {
+
+struct Context {
+  bool inited = false;
+  bool owns_memory = false;
+  void *base = nullptr;
+  size_t bytes = 0;
+  Geo g;
+  State8 U, Uh;
+  Flux21 F;
+  Edge3 E;
+  Scalars *sc = nullptr;
+  cudaStream_t stream = 0;
+  long long launches = 0;
+  bool graph_ok = false;
+};
+
+Context C;
+char g_err[512] = "no error";
+
+int fail(int code, const char *msg) {
+  snprintf(g_err, sizeof(g_err), "%s", msg);
+  return code;
+}
+
+int cuda_fail(cudaError_t e, const char *where) {
+  snprintf(g_err, sizeof(g_err), "CUDA error at %s: %s", where, cudaGetErrorString(e));
+  return MHD_ERR_CUDA;
+}
+
+#define CU(call)                                          \
+  do {                                                    \
+    cudaError_t e_ = (call);                              \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
+  } while (0)
+
+#define LAUNCH_CHECK(name)                                \
+  do {                                                    \
+    C.launches++;                                         \
+    cudaError_t e_ = cudaGetLastError();                  \
+    if (e_ != cudaSuccess) return cuda_fail(e_, name);    \
+  } while (0)
+
+inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+bool make_geo(Geo &g, int nx, int ny, int nz, double gamma, int recon) {
+  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || recon < 0 || recon > 2) return false;
+  g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
+  g.ng = 3 + recon;  // stencil radius: PCM 0, PLMC 1, PPMC 2
+  g.ox = round_up(g.ng, 4);
+  g.N[0] = round_up(g.ox + nx + g.ng, 8);
+  g.N[1] = ny + 2 * g.ng;
+  g.N[2] = nz + 2 * g.ng;
+  g.s[0] = 1; g.s[1] = g.N[0]; g.s[2] = (long long)g.N[0] * g.N[1];
+  g.ntot = g.s[2] * g.N[2];
+  for (int a = 0; a < 3; a++) { g.d[a] = 1.0 / g.n[a]; g.bc[a] = MHD_BC_PERIODIC; }
+  g.gamma = gamma;
+  g.recon = recon;
+  return true;
+}
+
+const int kNumArrays = 2 * NFIELD + 21 + 3;  // U, Uh, fluxes, edge fields
+
+size_t array_bytes(const Geo &g) { return ((size_t)g.ntot * sizeof(double) + 255) / 256 * 256; }
+
+size_t total_bytes(const Geo &g) { return array_bytes(g) * kNumArrays + 256; }
+
+dim3 grid1(long long n, int block) { return dim3((unsigned)((n + block - 1) / block)); }
+
+void extents(int f, const Geo &g, int &ex, int &ey, int &ez) {
+  ex = g.n[0] + (f == F_BX); ey = g.n[1] + (f == F_BY); ez = g.n[2] + (f == F_BZ);
+}
+
+int fill_ghosts(State8 &U) {
+  const Geo &g = C.g;
+  const int B = 256;
+  long long t0 = 2LL * g.ng * g.N[1] * g.N[2];
+  k_fill_ghosts<0><<<dim3(grid1(t0, B).x, 1, NFIELD), B, 0, C.stream>>>(U, g);
+  LAUNCH_CHECK("k_fill_ghosts<0>");
+  long long t1 = 2LL * g.ng * g.N[0] * g.N[2];
+  k_fill_ghosts<1><<<dim3(grid1(t1, B).x, 1, NFIELD), B, 0, C.stream>>>(U, g);
+  LAUNCH_CHECK("k_fill_ghosts<1>");
+  long long t2 = 2LL * g.ng * g.N[0] * g.N[1];
+  k_fill_ghosts<2><<<dim3(grid1(t2, B).x, 1, NFIELD), B, 0, C.stream>>>(U, g);
+  LAUNCH_CHECK("k_fill_ghosts<2>");
+  return MHD_OK;
+}
+
+Box make_box(int l0, int h0, int l1, int h1, int l2, int h2) {
+  Box b;
+  b.lo[0] = l0; b.hi[0] = h0; b.lo[1] = l1; b.hi[1] = h1; b.lo[2] = l2; b.hi[2] = h2;
+  return b;
+}
+
+template <int R>
+int launch_corrector_fluxes() {
+  const Geo &g = C.g;
+  const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
+  // faces 0..n along the sweep, transverse -1..n (what CT and the final update need)
+  {
+    Box fb = make_box(0, n0, -1, n1, -1, n2);
+    int ncell = n0 + 2;  // cells -1..n
+    dim3 grid((ncell - 1 + (MHD_BX - 1) - 1) / (MHD_BX - 1), n1 + 2, n2 + 2);
+    k_flux_x<R><<<grid, MHD_BX, 0, C.stream>>>(C.Uh, C.F, g, fb);
+    LAUNCH_CHECK("k_flux_x");
+  }
+  {
+    Box fb = make_box(-1, n0, 0, n1, -1, n2);
+    int J = (n1 + 1 >= 64) ? 32 : ((n1 + 1 >= 16) ? 8 : 4);
+    long long nt = (long long)(n0 + 2) * (n2 + 2);
+    dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
+    k_flux_march<1, R><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J);
+    LAUNCH_CHECK("k_flux_march<1>");
+  }
+  {
+    Box fb = make_box(-1, n0, -1, n1, 0, n2);
+    int J = (n2 + 1 >= 64) ? 32 : ((n2 + 1 >= 16) ? 8 : 4);
+    long long nt = (long long)(n0 + 2) * (n1 + 2);
+    dim3 grid(grid1(nt, 128).x, (n2 + 1 + J - 1) / J);
+    k_flux_march<2, R><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J);
+    LAUNCH_CHECK("k_flux_march<2>");
+  }
+  return MHD_OK;
+}
+
+// One VL+CT step with the dt held in C.sc->dt.
+int step_kernels() {
+  const Geo &g = C.g;
+  const int r = g.recon;
+  int rc = fill_ghosts(C.U);  // one boundary update per step
+  if (rc) return rc;
+  // Steps 2-3: PCM + HLLD on cells [-2-r, n+r+1]
+  Box pb;
+  for (int a = 0; a < 3; a++) { pb.lo[a] = -2 - r; pb.hi[a] = g.n[a] + r + 1; }
+  {
+    long long plane = (long long)(pb.hi[0] - pb.lo[0] + 1) * (pb.hi[1] - pb.lo[1] + 1);
+    dim3 grid(grid1(plane, 128).x, pb.hi[2] - pb.lo[2] + 1);
+    k_predictor_flux<<<grid, 128, 0, C.stream>>>(C.U, C.F, g, pb);
+    LAUNCH_CHECK("k_predictor_flux");
+  }
+  // Step 4: CT on indices [-1-r, n+r+1];  Step 5: half update of cells [-1-r, n+r]
+  Box hb;
+  for (int a = 0; a < 3; a++) { hb.lo[a] = -1 - r; hb.hi[a] = g.n[a] + r; }
+  {
+    Box eb = hb;
+    for (int a = 0; a < 3; a++) eb.hi[a] += 1;
+    long long plane = (long long)(eb.hi[0] - eb.lo[0] + 1) * (eb.hi[1] - eb.lo[1] + 1);
+    dim3 grid(grid1(plane, 128).x, eb.hi[2] - eb.lo[2] + 1);
+    k_ct<<<grid, 128, 0, C.stream>>>(C.U, C.F, C.E, g, eb);
+    LAUNCH_CHECK("k_ct(predictor)");
+    dim3 gridu(grid1(plane, 256).x, eb.hi[2] - eb.lo[2] + 1);
+    k_update<<<gridu, 256, 0, C.stream>>>(C.U, C.Uh, C.F, C.E, g, hb, C.sc, 0.5);
+    LAUNCH_CHECK("k_update(half)");
+  }
+  // Steps 6-7: reconstruction + HLLD from U^{n+1/2}
+  if (r == 0) rc = launch_corrector_fluxes<0>();
+  else if (r == 1) rc = launch_corrector_fluxes<1>();
+  else rc = launch_corrector_fluxes<2>();
+  if (rc) return rc;
+  // Step 8 (G12): CT with the corrector fluxes and the half-step reference state, indices [0, n]
+  // Step 9: full update of cells [0, n-1] and faces 0..n
+  {
+    Box ab, eb;
+    for (int a = 0; a < 3; a++) { ab.lo[a] = 0; ab.hi[a] = g.n[a] - 1; eb.lo[a] = 0; eb.hi[a] = g.n[a]; }
+    long long plane = (long long)(g.n[0] + 1) * (g.n[1] + 1);
+    dim3 grid(grid1(plane, 128).x, g.n[2] + 1);
+    k_ct<<<grid, 128, 0, C.stream>>>(C.Uh, C.F, C.E, g, eb);
+    LAUNCH_CHECK("k_ct(corrector)");
+    dim3 gridu(grid1(plane, 256).x, g.n[2] + 1);
+    k_update<<<gridu, 256, 0, C.stream>>>(C.U, C.U, C.F, C.E, g, ab, C.sc, 1.0);
+    LAUNCH_CHECK("k_update(full)");
+  }
+  return MHD_OK;
+}
+
+int cfl_kernel() {
+  const Geo &g = C.g;
+  long long plane = (long long)g.n[0] * g.n[1];
+  dim3 grid(grid1(plane, 256).x, g.n[2]);
+  k_cfl<<<grid, 256, 0, C.stream>>>(C.U, g, C.sc);
+  LAUNCH_CHECK("k_cfl");
+  return MHD_OK;
+}
+
+int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_t ws_bytes) {
+  mhd_finalize();
+  Geo g;
+  if (!make_geo(g, nx, ny, nz, gamma, recon)) return fail(MHD_ERR_ARG, "mhd_init: bad argument");
+  size_t need = total_bytes(g);
+  if (ws) {
+    if (ws_bytes < need || ((size_t)ws & 255)) return fail(MHD_ERR_NOMEM, "workspace too small or misaligned");
+    C.base = ws; C.owns_memory = false;
+  } else {
+    cudaError_t e = cudaMalloc(&C.base, need);
+    if (e != cudaSuccess) { cudaGetLastError(); C.base = nullptr; return fail(MHD_ERR_NOMEM, "cudaMalloc failed"); }
+    C.owns_memory = true;
+  }
+  C.bytes = need;
+  C.g = g;
+  char *p = (char *)C.base;
+  size_t ab = array_bytes(g);
+  C.sc = (Scalars *)p; p += 256;
+  for (int f = 0; f < NFIELD; f++) { C.U.f[f] = (double *)p; p += ab; }
+  for (int f = 0; f < NFIELD; f++) { C.Uh.f[f] = (double *)p; p += ab; }
+  for (int a = 0; a < 3; a++)
+    for (int c = 0; c < 7; c++) { C.F.f[a][c] = (double *)p; p += ab; }
+  for (int a = 0; a < 3; a++) { C.E.f[a] = (double *)p; p += ab; }
+  C.launches = 0;
+  C.inited = true;
+  cudaError_t e = cudaMemsetAsync(C.base, 0, need, C.stream);
+  if (e != cudaSuccess) { mhd_finalize(); return cuda_fail(e, "cudaMemsetAsync"); }
+  k_reset_min<<<1, 1, 0, C.stream>>>(C.sc);
+  LAUNCH_CHECK("k_reset_min");
+  return MHD_OK;
+}
+
+int set_state_from(const double *const src[NFIELD], bool host) {
+  const Geo &g = C.g;
+  for (int f = 0; f < NFIELD; f++)
+    if (!src[f]) return fail(MHD_ERR_ARG, "mhd_set_state: null pointer");
+  for (int f = 0; f < NFIELD; f++) {
+    int ex, ey, ez;
+    extents(f, g, ex, ey, ez);
+    long long cnt = (long long)ex * ey * ez;
+    const double *dsrc = src[f];
+    if (host) {  // stage through a flux array (free between steps)
+      double *stage = C.F.f[f / 7][f % 7];
+      CU(cudaMemcpyAsync(stage, src[f], cnt * sizeof(double), cudaMemcpyHostToDevice, C.stream));
+      dsrc = stage;
+    }
+    k_unpack<<<grid1(cnt, 256), 256, 0, C.stream>>>(C.U.f[f], dsrc, g, ex, ey, ez);
+    LAUNCH_CHECK("k_unpack");
+  }
+  return fill_ghosts(C.U);
+}
+
+int get_state_to(State8 &S, double *const dst[NFIELD], bool host) {
+  const Geo &g = C.g;
+  for (int f = 0; f < NFIELD; f++) {
+    if (!dst[f]) continue;
+    int ex, ey, ez;
+    extents(f, g, ex, ey, ez);
+    long long cnt = (long long)ex * ey * ez;
+    double *ddst = host ? C.F.f[f / 7][f % 7] : dst[f];
+    k_pack<<<grid1(cnt, 256), 256, 0, C.stream>>>(ddst, S.f[f], g, ex, ey, ez);
+    LAUNCH_CHECK("k_pack");
+    if (host) CU(cudaMemcpyAsync(dst[f], ddst, cnt * sizeof(double), cudaMemcpyDeviceToHost, C.stream));
+  }
+  return MHD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t mhd_workspace_bytes(int nx, int ny, int nz, int recon) {
+  Geo g;
+  if (!make_geo(g, nx, ny, nz, 1.5, recon)) return 0;
+  return total_bytes(g);
+}
+
+int mhd_init(int nx, int ny, int nz, double gamma, int recon) {
+  return init_common(nx, ny, nz, gamma, recon, nullptr, 0);
+}
+
+int mhd_init_workspace(int nx, int ny, int nz, double gamma, int recon, void *workspace,
+                       size_t workspace_bytes) {
+  if (!workspace) return fail(MHD_ERR_ARG, "mhd_init_workspace: null workspace");
+  return init_common(nx, ny, nz, gamma, recon, workspace, workspace_bytes);
+}
+
+int mhd_set_boundary(int axis, int kind) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (axis < 0 || axis > 2 || (kind != MHD_BC_PERIODIC && kind != MHD_BC_OUTFLOW))
+    return fail(MHD_ERR_ARG, "mhd_set_boundary: bad argument");
+  C.g.bc[axis] = kind;
+  return MHD_OK;
+}
+
+int mhd_set_stream(void *cuda_stream) {
+  C.stream = (cudaStream_t)cuda_stream;
+  return MHD_OK;
+}
+
+int mhd_set_state(const double *rho, const double *mx, const double *my, const double *mz,
+                  const double *E, const double *bx, const double *by, const double *bz) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  const double *src[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
+  int rc = set_state_from(src, true);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(C.stream));
+  return MHD_OK;
+}
+
+int mhd_set_state_device(const double *rho, const double *mx, const double *my, const double *mz,
+                         const double *E, const double *bx, const double *by, const double *bz) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  const double *src[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
+  return set_state_from(src, false);
+}
+
+int mhd_compute_dt(double cfl, double *dt) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (!dt || !(cfl > 0.0)) return fail(MHD_ERR_ARG, "mhd_compute_dt: bad argument");
+  int rc = cfl_kernel();
+  if (rc) return rc;
+  Scalars h;
+  CU(cudaMemcpyAsync(&h, C.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, C.stream));
+  k_reset_min<<<1, 1, 0, C.stream>>>(C.sc);
+  LAUNCH_CHECK("k_reset_min");
+  CU(cudaStreamSynchronize(C.stream));
+  double m;
+  memcpy(&m, &h.min_bits, sizeof(double));
+  *dt = cfl * m;
+  if (h.bad) return fail(MHD_ERR_UNPHYSICAL, "non-physical state (rho <= 0, P <= 0 or non-finite)");
+  return MHD_OK;
+}
+
+int mhd_step(double dt) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (!(dt > 0.0)) return fail(MHD_ERR_ARG, "mhd_step: dt must be positive");
+  k_set_dt<<<1, 1, 0, C.stream>>>(C.sc, dt);
+  LAUNCH_CHECK("k_set_dt");
+  return step_kernels();
+}
+
+int mhd_advance(int n_steps, double cfl, double *t_accum) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (n_steps < 0 || !(cfl > 0.0)) return fail(MHD_ERR_ARG, "mhd_advance: bad argument");
+  Scalars h;
+  double t0 = 0.0;
+  if (t_accum) {
+    CU(cudaMemcpyAsync(&h, C.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, C.stream));
+    CU(cudaStreamSynchronize(C.stream));
+    t0 = h.t_accum;
+  }
+  for (int s = 0; s < n_steps; s++) {
+    int rc = cfl_kernel();
+    if (rc) return rc;
+    k_finish_dt<<<1, 1, 0, C.stream>>>(C.sc, cfl);
+    LAUNCH_CHECK("k_finish_dt");
+    rc = step_kernels();
+    if (rc) return rc;
+  }
+  if (t_accum) {
+    CU(cudaMemcpyAsync(&h, C.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, C.stream));
+    CU(cudaStreamSynchronize(C.stream));
+    *t_accum = h.t_accum - t0;
+    if (h.bad) return fail(MHD_ERR_UNPHYSICAL, "non-physical state (rho <= 0, P <= 0 or non-finite)");
+  }
+  return MHD_OK;
+}
+
+int mhd_get_state(double *rho, double *mx, double *my, double *mz, double *E, double *bx,
+                  double *by, double *bz) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  double *dst[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
+  int rc = get_state_to(C.U, dst, true);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(C.stream));
+  return MHD_OK;
+}
+
+int mhd_get_state_device(double *rho, double *mx, double *my, double *mz, double *E, double *bx,
+                         double *by, double *bz) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  double *dst[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
+  return get_state_to(C.U, dst, false);
+}
+
+int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *E, double *bx,
+                       double *by, double *bz) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  double *dst[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
+  int rc = get_state_to(C.Uh, dst, true);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(C.stream));
+  return MHD_OK;
+}
+
+int mhd_max_divb(double *out) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (!out) return fail(MHD_ERR_ARG, "mhd_max_divb: null pointer");
+  const Geo &g = C.g;
+  unsigned long long *bits = (unsigned long long *)C.E.f[0];  // edge fields are free between steps
+  CU(cudaMemsetAsync(bits, 0, sizeof(unsigned long long), C.stream));
+  long long plane = (long long)g.n[0] * g.n[1];
+  dim3 grid(grid1(plane, 256).x, g.n[2]);
+  k_divb<<<grid, 256, 0, C.stream>>>(C.U, g, bits);
+  LAUNCH_CHECK("k_divb");
+  unsigned long long h;
+  CU(cudaMemcpyAsync(&h, bits, sizeof(h), cudaMemcpyDeviceToHost, C.stream));
+  CU(cudaStreamSynchronize(C.stream));
+  memcpy(out, &h, sizeof(double));
+  return MHD_OK;
+}
+
+long long mhd_launch_count(void) { return C.launches; }
+
+int mhd_synchronize(void) {
+  CU(cudaStreamSynchronize(C.stream));
+  return MHD_OK;
+}
+
+int mhd_finalize(void) {
+  if (C.inited) {
+    cudaStreamSynchronize(C.stream);
+    if (C.owns_memory && C.base) cudaFree(C.base);
+  }
+  cudaStream_t s = C.stream;
+  C = Context();
+  C.stream = s;
+  return MHD_OK;
+}
+
+const char *mhd_last_error(void) { return g_err; }
+
+}  // extern "C"

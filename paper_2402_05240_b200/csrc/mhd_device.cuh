@@ -1,0 +1,377 @@
+// mhd_device.cuh -- per-cell / per-face device arithmetic of the VL+CT step (sm_100a, fp64).
+//
+// Everything here is register-resident scalar code, written from the paper
+// (/root/reference/PAPER.md, cited as PAPER.md:<line>) and the readings O0..O12 listed in
+// DESIGN.md.  No fast-math; FMA contraction is left to nvcc (default --fmad=true).
+// Solver-local 1-D state for a sweep along axis a (O0): W = (rho, u, v, w, P, By, Bz) with
+// (u,v,w) = (v_a, v_{a+1}, v_{a+2}), (By,Bz) = (B_{a+1}, B_{a+2}) (indices mod 3); the normal
+// field Bn is carried separately.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace mhd {
+
+struct W7 {
+  double rho, u, v, w, P, by, bz;
+};
+
+struct F7 {  // mass, mom_n, mom_t1, mom_t2, energy, By-flux, Bz-flux
+  double m, mn, mt1, mt2, e, by, bz;
+};
+
+// Eq. 12: c_f^2 along the direction whose field component is bn.
+// The discriminant is clamped at 0 against round-off (reading R3).
+__device__ __forceinline__ double fast_speed_sq(double gamma, double rho, double P, double bn,
+                                                double bt1, double bt2) {
+  double gp = gamma * P;
+  double b2 = bn * bn + bt1 * bt1 + bt2 * bt2;
+  double s = gp + b2;
+  double disc = s * s - 4.0 * gp * bn * bn;
+  disc = disc < 0.0 ? 0.0 : disc;
+  return (s + sqrt(disc)) / (2.0 * rho);
+}
+
+// ---------------------------------------------------------------------------------------
+// HLLD (Miyoshi & Kusano 2005, cited PAPER.md:149; reading O4, wave speeds G15).
+// ---------------------------------------------------------------------------------------
+struct HlldSide {
+  double rho, u, v, w, by, bz;  // primitive inputs
+  double pT, e;                 // total pressure, total energy density
+  double Fm, Fmn, Fmt1, Fmt2, Fe, Fby, Fbz;  // physical flux, Eq. 8
+  double rhos, vs, ws, bys, bzs, es;         // single-star state
+};
+
+__device__ __forceinline__ void hlld_side_init(HlldSide &s, const W7 &W, double bx, double gm1inv,
+                                               double &P) {
+  s.rho = W.rho; s.u = W.u; s.v = W.v; s.w = W.w; s.by = W.by; s.bz = W.bz; P = W.P;
+  double b2 = bx * bx + W.by * W.by + W.bz * W.bz;
+  s.pT = W.P + 0.5 * b2;
+  s.e = W.P * gm1inv + 0.5 * W.rho * (W.u * W.u + W.v * W.v + W.w * W.w) + 0.5 * b2;
+  s.Fm = W.rho * W.u;
+  s.Fmn = W.rho * W.u * W.u + s.pT - bx * bx;
+  s.Fmt1 = W.rho * W.u * W.v - bx * W.by;
+  s.Fmt2 = W.rho * W.u * W.w - bx * W.bz;
+  s.Fe = W.u * (s.e + s.pT) - bx * (W.u * bx + W.v * W.by + W.w * W.bz);
+  s.Fby = W.by * W.u - bx * W.v;
+  s.Fbz = W.bz * W.u - bx * W.w;
+}
+
+// single-star state of one side (M&K Eq. 43-48); S = outer speed of this side
+__device__ __forceinline__ void hlld_star(HlldSide &s, double S, double SM, double pTs, double bx) {
+  double Su = S - s.u;
+  double SSm = S - SM;
+  double iSSm = 1.0 / SSm;
+  s.rhos = s.rho * (Su * iSSm);
+  double D = s.rho * Su * SSm - bx * bx;
+  if (fabs(D) < 1e-8 * pTs) {  // degenerate 0/0: no jump in the tangential fields
+    s.vs = s.v; s.ws = s.w; s.bys = s.by; s.bzs = s.bz;
+  } else {
+    double iD = 1.0 / D;
+    double fv = bx * (SM - s.u) * iD;
+    double fb = (s.rho * Su * Su - bx * bx) * iD;
+    s.vs = s.v - s.by * fv;
+    s.ws = s.w - s.bz * fv;
+    s.bys = s.by * fb;
+    s.bzs = s.bz * fb;
+  }
+  double vb = s.u * bx + s.v * s.by + s.w * s.bz;
+  double vbs = SM * bx + s.vs * s.bys + s.ws * s.bzs;
+  s.es = (Su * s.e - s.pT * s.u + pTs * SM + bx * (vb - vbs)) * iSSm;
+}
+
+__device__ __forceinline__ F7 hlld(double gamma, const W7 &WL, const W7 &WR, double bx) {
+  HlldSide L, R;
+  double PL, PR;
+  double gm1inv = 1.0 / (gamma - 1.0);
+  hlld_side_init(L, WL, bx, gm1inv, PL);
+  hlld_side_init(R, WR, bx, gm1inv, PR);
+  double cfL = sqrt(fast_speed_sq(gamma, L.rho, PL, bx, L.by, L.bz));
+  double cfR = sqrt(fast_speed_sq(gamma, R.rho, PR, bx, R.by, R.bz));
+  double cfmax = fmax(cfL, cfR);
+  double SL = fmin(L.u, R.u) - cfmax;
+  double SR = fmax(L.u, R.u) + cfmax;
+
+  F7 F;
+  if (SL > 0.0) {
+    F.m = L.Fm; F.mn = L.Fmn; F.mt1 = L.Fmt1; F.mt2 = L.Fmt2; F.e = L.Fe; F.by = L.Fby; F.bz = L.Fbz;
+    return F;
+  }
+  if (SR < 0.0) {
+    F.m = R.Fm; F.mn = R.Fmn; F.mt1 = R.Fmt1; F.mt2 = R.Fmt2; F.e = R.Fe; F.by = R.Fby; F.bz = R.Fbz;
+    return F;
+  }
+  // middle wave and total pressure of the fan (M&K Eq. 38, 41)
+  double sduL = (SL - L.u) * L.rho;
+  double sduR = (SR - R.u) * R.rho;
+  double iden = 1.0 / (sduR - sduL);
+  double SM = (sduR * R.u - sduL * L.u - R.pT + L.pT) * iden;
+  double pTs = (sduR * L.pT - sduL * R.pT + L.rho * R.rho * (SR - R.u) * (SL - L.u) * (R.u - L.u)) * iden;
+
+  hlld_star(L, SL, SM, pTs, bx);
+  hlld_star(R, SR, SM, pTs, bx);
+  double rL = sqrt(L.rhos), rR = sqrt(R.rhos);
+  double abx = fabs(bx);
+  double SsL = SM - abx / rL;
+  double SsR = SM + abx / rR;
+
+  // side whose states bound the face: left if S_M >= 0 (S*_L >= 0 implies S_M >= 0)
+  bool left = (SM >= 0.0);
+  bool dbl = left ? !(SsL >= 0.0) : !(SsR <= 0.0);
+  const HlldSide &a = left ? L : R;
+  double S = left ? SL : SR;
+  double Ss = left ? SsL : SsR;
+  double Um = a.rho, Umn = a.rho * a.u, Umt1 = a.rho * a.v, Umt2 = a.rho * a.w;
+  double Usm = a.rhos, Usmn = a.rhos * SM, Usmt1 = a.rhos * a.vs, Usmt2 = a.rhos * a.ws;
+  // F*_a = F_a + S_a (U*_a - U_a)
+  F.m = a.Fm + S * (Usm - Um);
+  F.mn = a.Fmn + S * (Usmn - Umn);
+  F.mt1 = a.Fmt1 + S * (Usmt1 - Umt1);
+  F.mt2 = a.Fmt2 + S * (Usmt2 - Umt2);
+  F.e = a.Fe + S * (a.es - a.e);
+  F.by = a.Fby + S * (a.bys - a.by);
+  F.bz = a.Fbz + S * (a.bzs - a.bz);
+  if (dbl) {
+    // double-star states (M&K Eq. 59-63)
+    double sgn = (bx > 0.0) ? 1.0 : ((bx < 0.0) ? -1.0 : 0.0);
+    double inv = 1.0 / (rL + rR);
+    double vss = (rL * L.vs + rR * R.vs + (R.bys - L.bys) * sgn) * inv;
+    double wss = (rL * L.ws + rR * R.ws + (R.bzs - L.bzs) * sgn) * inv;
+    double byss = (rL * R.bys + rR * L.bys + rL * rR * (R.vs - L.vs) * sgn) * inv;
+    double bzss = (rL * R.bzs + rR * L.bzs + rL * rR * (R.ws - L.ws) * sgn) * inv;
+    double vbss = SM * bx + vss * byss + wss * bzss;
+    double vbs = SM * bx + a.vs * a.bys + a.ws * a.bzs;
+    double r = left ? rL : rR;
+    double ess = left ? a.es - r * (vbs - vbss) * sgn : a.es + r * (vbs - vbss) * sgn;
+    // F**_a = F*_a + S*_a (U**_a - U*_a); rho** = rho*, u** = S_M
+    F.mt1 += Ss * (a.rhos * vss - Usmt1);
+    F.mt2 += Ss * (a.rhos * wss - Usmt2);
+    F.e += Ss * (ess - a.es);
+    F.by += Ss * (byss - a.bys);
+    F.bz += Ss * (bzss - a.bzs);
+    // mass and normal momentum: U** - U* = 0 exactly
+  }
+  return F;
+}
+
+// ---------------------------------------------------------------------------------------
+// Eigen-system of the primitive-variable equations (Stone et al. 2008 App. A, cited
+// PAPER.md:249; reading O9, degenerate normalisation G16), held as the dozen scalars the
+// 7x7 matrices are built from.  Wave order u-cf, u-ca, u-cs, u, u+cs, u+ca, u+cf.
+// The left/right projections below are the matrix-vector products L.x and R.a written out
+// with the structural zeros removed and the transverse components rotated into the
+// (parallel, perpendicular)-to-B_perp frame: xp = by*X_y + bz*X_z, xq = by*X_z - bz*X_y.
+// ---------------------------------------------------------------------------------------
+struct Eig {
+  double rho, irho, a2, ia2, N;
+  double betay, betaz, alf, als;
+  double Cff, Css, Qf, Qs, Af, As;
+  double Ssr;   // S * sqrt(rho)
+  double Sisr;  // S / sqrt(rho)
+};
+
+struct C7 {  // characteristic amplitudes
+  double c0, c1, c2, c3, c4, c5, c6;
+};
+
+__device__ __forceinline__ void eig_setup(Eig &e, double gamma, const W7 &W, double bx) {
+  double rho = W.rho;
+  double irho = 1.0 / rho;
+  double a2 = gamma * W.P * irho;
+  double a = sqrt(a2);
+  double cf2 = fast_speed_sq(gamma, rho, W.P, bx, W.by, W.bz);
+  double ca2 = bx * bx * irho;
+  double cs2 = (cf2 > 0.0) ? a2 * ca2 / cf2 : 0.0;
+  double cf = sqrt(cf2), cs = sqrt(cs2);
+  double bperp = sqrt(W.by * W.by + W.bz * W.bz);
+  if (bperp == 0.0) { e.betay = 1.0; e.betaz = 0.0; }
+  else { double ib = 1.0 / bperp; e.betay = W.by * ib; e.betaz = W.bz * ib; }
+  double dfs = cf2 - cs2;
+  if (dfs == 0.0) { e.alf = 1.0; e.als = 0.0; }
+  else {
+    double idfs = 1.0 / dfs;
+    double af2 = (a2 - cs2) * idfs;
+    double as2 = (cf2 - a2) * idfs;
+    af2 = af2 < 0.0 ? 0.0 : (af2 > 1.0 ? 1.0 : af2);
+    as2 = as2 < 0.0 ? 0.0 : (as2 > 1.0 ? 1.0 : as2);
+    e.alf = sqrt(af2); e.als = sqrt(as2);
+  }
+  double S = (bx >= 0.0) ? 1.0 : -1.0;
+  double sr = sqrt(rho);
+  e.rho = rho; e.irho = irho; e.a2 = a2; e.ia2 = 1.0 / a2; e.N = 0.5 * e.ia2;
+  e.Cff = cf * e.alf; e.Css = cs * e.als;
+  e.Qf = e.Cff * S; e.Qs = e.Css * S;
+  e.Af = a * e.alf * sr; e.As = a * e.als * sr;
+  e.Ssr = S * sr; e.Sisr = S / sr;
+}
+
+// a = L . x   (x in the component order of W7)
+__device__ __forceinline__ C7 eig_left(const Eig &e, const W7 &x) {
+  double xp = e.betay * x.v + e.betaz * x.w;
+  double xq = e.betay * x.w - e.betaz * x.v;
+  double bp = e.betay * x.by + e.betaz * x.bz;
+  double bq = e.betay * x.bz - e.betaz * x.by;
+  double f1 = e.Cff * x.u - e.Qs * xp;
+  double f2 = (e.alf * x.P + e.As * bp) * e.irho;
+  double s1 = e.Css * x.u + e.Qf * xp;
+  double s2 = (e.als * x.P - e.Af * bp) * e.irho;
+  double q2 = e.Sisr * bq;
+  C7 c;
+  c.c0 = e.N * (f2 - f1);
+  c.c6 = e.N * (f2 + f1);
+  c.c2 = e.N * (s2 - s1);
+  c.c4 = e.N * (s2 + s1);
+  c.c1 = 0.5 * (q2 + xq);
+  c.c5 = 0.5 * (q2 - xq);
+  c.c3 = x.rho - x.P * e.ia2;
+  return c;
+}
+
+// x = R . a
+__device__ __forceinline__ W7 eig_right(const Eig &e, const C7 &c) {
+  double fs = c.c0 + c.c6, fd = c.c6 - c.c0;
+  double ss = c.c2 + c.c4, sd = c.c4 - c.c2;
+  double as_ = c.c1 + c.c5, ad = c.c1 - c.c5;
+  double comp = e.alf * fs + e.als * ss;
+  double tp = e.Qf * sd - e.Qs * fd;   // transverse velocity along B_perp
+  double bp = e.As * fs - e.Af * ss;   // transverse field along B_perp
+  double bq = e.Ssr * as_;             // transverse field across B_perp
+  W7 x;
+  x.rho = e.rho * comp + c.c3;
+  x.u = e.Cff * fd + e.Css * sd;
+  x.v = e.betay * tp - e.betaz * ad;
+  x.w = e.betaz * tp + e.betay * ad;
+  x.P = e.rho * e.a2 * comp;
+  x.by = e.betay * bp - e.betaz * bq;
+  x.bz = e.betaz * bp + e.betay * bq;
+  return x;
+}
+
+// ---------------------------------------------------------------------------------------
+// PLMC, Eq. 23-28 (reading O8).  Out: Wlo = W_{R,i-1/2}, Whi = W_{L,i+1/2}.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double vl_slope(double dl, double dr) {  // Eq. 26 (G10)
+  return (dl * dr > 0.0) ? 2.0 * dl * dr / (dl + dr) : 0.0;
+}
+
+__device__ __forceinline__ double plm_limit(double aL, double aR, double aC, double aVL) {  // Eq. 27
+  if (aL * aR > 0.0) {
+    double m = fmin(fmin(2.0 * fabs(aL), 2.0 * fabs(aR)), fmin(fabs(aC), fabs(aVL)));
+    return (aC > 0.0) ? m : ((aC < 0.0) ? -m : 0.0);
+  }
+  return 0.0;
+}
+
+__device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, const W7 &Wp,
+                                     double bx0, W7 &Wlo, W7 &Whi) {
+  Eig e;
+  eig_setup(e, gamma, W0, bx0);
+  W7 dL, dR, dC, dV;
+#define MHD_D4(f)                                   \
+  dL.f = W0.f - Wm.f; dR.f = Wp.f - W0.f;           \
+  dC.f = (Wp.f - Wm.f) / 2.0; dV.f = vl_slope(dL.f, dR.f);
+  MHD_D4(rho) MHD_D4(u) MHD_D4(v) MHD_D4(w) MHD_D4(P) MHD_D4(by) MHD_D4(bz)
+#undef MHD_D4
+  C7 aL = eig_left(e, dL), aR = eig_left(e, dR), aC = eig_left(e, dC), aV = eig_left(e, dV);
+  C7 am;
+  am.c0 = plm_limit(aL.c0, aR.c0, aC.c0, aV.c0);
+  am.c1 = plm_limit(aL.c1, aR.c1, aC.c1, aV.c1);
+  am.c2 = plm_limit(aL.c2, aR.c2, aC.c2, aV.c2);
+  am.c3 = plm_limit(aL.c3, aR.c3, aC.c3, aV.c3);
+  am.c4 = plm_limit(aL.c4, aR.c4, aC.c4, aV.c4);
+  am.c5 = plm_limit(aL.c5, aR.c5, aC.c5, aV.c5);
+  am.c6 = plm_limit(aL.c6, aR.c6, aC.c6, aV.c6);
+  W7 dW = eig_right(e, am);
+#define MHD_O(f) Whi.f = W0.f + dW.f / 2.0; Wlo.f = W0.f - dW.f / 2.0;
+  MHD_O(rho) MHD_O(u) MHD_O(v) MHD_O(w) MHD_O(P) MHD_O(by) MHD_O(bz)
+#undef MHD_O
+}
+
+// ---------------------------------------------------------------------------------------
+// PPMC (reading O10 / G17 of Felker & Stone 2018, cited PAPER.md:231, 431).
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double sgn3(double x) { return (x > 0.0) ? 1.0 : ((x < 0.0) ? -1.0 : 0.0); }
+
+// limited 4th-order value on the face between cells j and j+1; qa..qd = q_{j-1..j+2}
+__device__ __forceinline__ double ppm_face(double qa, double qb, double qc, double qd) {
+  const double C = 1.25;
+  double qf = (7.0 / 12.0) * (qb + qc) - (1.0 / 12.0) * (qa + qd);
+  if ((qf - qb) * (qc - qf) < 0.0) {
+    double Df = 3.0 * (qb - 2.0 * qf + qc);
+    double Dj = qa - 2.0 * qb + qc;
+    double Dj1 = qb - 2.0 * qc + qd;
+    double s = sgn3(Df);
+    double Dlim = 0.0;
+    if (s != 0.0 && s == sgn3(Dj) && s == sgn3(Dj1))
+      Dlim = s * fmin(fmin(C * fabs(Dj), C * fabs(Dj1)), fabs(Df));
+    qf = 0.5 * (qb + qc) - Dlim / 6.0;
+  }
+  return qf;
+}
+
+__device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, double q3, double q4,
+                                           double &qlo, double &qhi) {
+  const double C = 1.25;
+  double qm = ppm_face(q0, q1, q2, q3);
+  double qp = ppm_face(q1, q2, q3, q4);
+  double qi = q2;
+  double dm = qi - qm, dp = qp - qi;
+  if (dm * dp <= 0.0 || (q3 - qi) * (qi - q1) <= 0.0) {
+    double Df = 6.0 * (qm - 2.0 * qi + qp);
+    double Dm1 = q0 - 2.0 * q1 + q2;
+    double D0 = q1 - 2.0 * q2 + q3;
+    double Dp1 = q2 - 2.0 * q3 + q4;
+    double Dlim = 0.0, r = 0.0;
+    double s = sgn3(Df);
+    if (s != 0.0 && s == sgn3(Dm1) && s == sgn3(D0) && s == sgn3(Dp1))
+      Dlim = s * fmin(fmin(C * fabs(Dm1), C * fabs(D0)), fmin(C * fabs(Dp1), fabs(Df)));
+    if (fabs(Df) > 1e-12 * fmax(fabs(q1), fmax(fabs(q2), fabs(q3)))) r = Dlim / Df;
+    if (r <= 1.0 - 1e-12) { qm = qi - r * dm; qp = qi + r * dp; }
+  } else {
+    if (fabs(dm) >= 2.0 * fabs(dp)) qm = qi - 2.0 * dp;
+    if (fabs(dp) >= 2.0 * fabs(dm)) qp = qi + 2.0 * dm;
+  }
+  qlo = qm; qhi = qp;
+}
+
+// Wm2..Wp2 = W_{i-2..i+2}; bx0 = cell-centred normal field of cell i
+__device__ __forceinline__ void ppmc(double gamma, const W7 &Wm2, const W7 &Wm1, const W7 &W0,
+                                     const W7 &Wp1, const W7 &Wp2, double bx0, W7 &Wlo, W7 &Whi) {
+  Eig e;
+  eig_setup(e, gamma, W0, bx0);
+  C7 q0 = eig_left(e, Wm2), q1 = eig_left(e, Wm1), q2 = eig_left(e, W0), q3 = eig_left(e, Wp1),
+     q4 = eig_left(e, Wp2);
+  C7 lo, hi;
+  ppm_scalar(q0.c0, q1.c0, q2.c0, q3.c0, q4.c0, lo.c0, hi.c0);
+  ppm_scalar(q0.c1, q1.c1, q2.c1, q3.c1, q4.c1, lo.c1, hi.c1);
+  ppm_scalar(q0.c2, q1.c2, q2.c2, q3.c2, q4.c2, lo.c2, hi.c2);
+  ppm_scalar(q0.c3, q1.c3, q2.c3, q3.c3, q4.c3, lo.c3, hi.c3);
+  ppm_scalar(q0.c4, q1.c4, q2.c4, q3.c4, q4.c4, lo.c4, hi.c4);
+  ppm_scalar(q0.c5, q1.c5, q2.c5, q3.c5, q4.c5, lo.c5, hi.c5);
+  ppm_scalar(q0.c6, q1.c6, q2.c6, q3.c6, q4.c6, lo.c6, hi.c6);
+  Wlo = eig_right(e, lo);
+  Whi = eig_right(e, hi);
+}
+
+// ---------------------------------------------------------------------------------------
+// CT edge field, Eq. 15-18 (readings O6, G5-G7).  Edge along c at
+// (ia-1/2, ib-1/2), (a,b,c) cyclic.  Ea0/Ea1 = E_c on the a-faces (ia-1/2, ib) / (ia-1/2, ib-1);
+// Eb0/Eb1 = E_c on the b-faces (ia, ib-1/2) / (ia-1, ib-1/2); M* the mass fluxes on those
+// faces; Er00, Er10, Er01, Er11 = reference field of cells (ia,ib), (ia-1,ib), (ia,ib-1),
+// (ia-1,ib-1).  All Delta factors of Eq. 15 and 17 cancel.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double upwind(double M, double from_lower, double from_upper) {
+  return (M > 0.0) ? from_lower : ((M < 0.0) ? from_upper : 0.5 * (from_lower + from_upper));
+}
+
+__device__ __forceinline__ double ct_edge(double Ea0, double Ea1, double Eb0, double Eb1, double Ma0,
+                                          double Ma1, double Mb0, double Mb1, double Er00,
+                                          double Er10, double Er01, double Er11) {
+  double T1 = upwind(Ma0, Eb1 - Er10, Eb0 - Er00);
+  double T2 = upwind(Ma1, Eb1 - Er11, Eb0 - Er01);
+  double T3 = upwind(Mb0, Ea1 - Er01, Ea0 - Er00);
+  double T4 = upwind(Mb1, Ea1 - Er11, Ea0 - Er10);
+  return 0.25 * (Ea0 + Ea1 + Eb0 + Eb1) + 0.25 * (T1 + T2 + T3 + T4);
+}
+
+}  // namespace mhd

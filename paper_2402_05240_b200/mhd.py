@@ -1,0 +1,177 @@
+"""Thin ctypes binding of libmhd.so (include/mhd.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used for
+device memory (the workspace tensor, device-resident input/output tensors) and streams.
+There is no CPU fallback: importing this module raises if the library is missing, and every
+call raises MhdError on a non-zero return code.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from .inputs import FIELDS, field_shapes
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmhd.so")
+
+RECON_PCM, RECON_PLMC, RECON_PPMC = 0, 1, 2
+BC_PERIODIC, BC_OUTFLOW = 0, 1
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_vp = ctypes.c_void_p
+
+
+class MhdError(RuntimeError):
+    pass
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "%s not found: build it with `python -m paper_2402_05240_b200.build` "
+            "(there is no CPU fallback)" % LIB_PATH)
+    L = ctypes.CDLL(LIB_PATH)
+    L.mhd_workspace_bytes.argtypes = [ctypes.c_int] * 4
+    L.mhd_workspace_bytes.restype = ctypes.c_size_t
+    L.mhd_init.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double, ctypes.c_int]
+    L.mhd_init_workspace.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double, ctypes.c_int, _vp, ctypes.c_size_t]
+    L.mhd_set_boundary.argtypes = [ctypes.c_int, ctypes.c_int]
+    L.mhd_set_stream.argtypes = [_vp]
+    L.mhd_set_state.argtypes = [_dp] * 8
+    L.mhd_set_state_device.argtypes = [_vp] * 8
+    L.mhd_compute_dt.argtypes = [ctypes.c_double, _dp]
+    L.mhd_step.argtypes = [ctypes.c_double]
+    L.mhd_advance.argtypes = [ctypes.c_int, ctypes.c_double, _dp]
+    L.mhd_get_state.argtypes = [_dp] * 8
+    L.mhd_get_state_device.argtypes = [_vp] * 8
+    L.mhd_get_half_state.argtypes = [_dp] * 8
+    L.mhd_max_divb.argtypes = [_dp]
+    L.mhd_launch_count.restype = ctypes.c_longlong
+    L.mhd_last_error.restype = ctypes.c_char_p
+    for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_stream", "mhd_set_state",
+                 "mhd_set_state_device", "mhd_compute_dt", "mhd_step", "mhd_advance", "mhd_get_state",
+                 "mhd_get_state_device", "mhd_get_half_state", "mhd_max_divb", "mhd_synchronize",
+                 "mhd_finalize"):
+        getattr(L, name).restype = ctypes.c_int
+    return L
+
+
+_lib = _load()
+
+
+def lib():
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise MhdError("libmhd error %d: %s" % (rc, _lib.mhd_last_error().decode()))
+
+
+def _hp(a):
+    return a.ctypes.data_as(_dp)
+
+
+class Mhd:
+    """The single global context of libmhd.so, same call sequence as the C ABI."""
+
+    def __init__(self, nx, ny, nz, gamma, recon=RECON_PLMC, bc=(0, 0, 0), use_torch_workspace=True,
+                 stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise MhdError("no CUDA device: the VL+CT step has no CPU fallback")
+        self.n = (nx, ny, nz)
+        self.recon = recon
+        self._torch = torch
+        self._ws = None
+        if stream is not None:
+            _check(_lib.mhd_set_stream(_vp(stream.cuda_stream)))
+        else:
+            _check(_lib.mhd_set_stream(None))
+        if use_torch_workspace:
+            nbytes = _lib.mhd_workspace_bytes(nx, ny, nz, recon)
+            if nbytes == 0:
+                raise MhdError("bad grid arguments")
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+            ptr = (self._ws.data_ptr() + 255) // 256 * 256
+            _check(_lib.mhd_init_workspace(nx, ny, nz, float(gamma), int(recon), _vp(ptr), nbytes))
+        else:
+            _check(_lib.mhd_init(nx, ny, nz, float(gamma), int(recon)))
+        for a, kind in enumerate(bc):
+            _check(_lib.mhd_set_boundary(a, int(kind)))
+
+    # ---- host-buffer path -------------------------------------------------------------
+    def set_state(self, state):
+        sh = field_shapes(*self.n)
+        arrs = []
+        for f in FIELDS:
+            a = np.ascontiguousarray(state[f], dtype=np.float64)
+            if a.shape != sh[f]:
+                raise MhdError("field %s has shape %s, expected %s" % (f, a.shape, sh[f]))
+            arrs.append(a)
+        _check(_lib.mhd_set_state(*[_hp(a) for a in arrs]))
+
+    def _get_host(self, fn, out=None):
+        sh = field_shapes(*self.n)
+        if out is None:
+            out = {f: np.empty(sh[f]) for f in FIELDS}
+        _check(fn(*[_hp(out[f]) for f in FIELDS]))
+        return out
+
+    def get_state(self, out=None):
+        return self._get_host(_lib.mhd_get_state, out)
+
+    def get_half_state(self):
+        return self._get_host(_lib.mhd_get_half_state)
+
+    # ---- device-buffer path -----------------------------------------------------------
+    def set_state_device(self, tensors):
+        """tensors: dict of 8 contiguous float64 CUDA tensors in the ABI layout."""
+        self._check_dev(tensors)
+        _check(_lib.mhd_set_state_device(*[_vp(tensors[f].data_ptr()) for f in FIELDS]))
+
+    def get_state_device(self, tensors):
+        self._check_dev(tensors)
+        _check(_lib.mhd_get_state_device(*[_vp(tensors[f].data_ptr()) for f in FIELDS]))
+        return tensors
+
+    def _check_dev(self, tensors):
+        sh = field_shapes(*self.n)
+        for f in FIELDS:
+            t = tensors[f]
+            if (not t.is_cuda or t.dtype != self._torch.float64 or not t.is_contiguous()
+                    or tuple(t.shape) != sh[f]):
+                raise MhdError("field %s: need a contiguous float64 CUDA tensor of shape %s" % (f, sh[f]))
+
+    # ---- the hot path -----------------------------------------------------------------
+    def compute_dt(self, cfl):
+        dt = ctypes.c_double()
+        _check(_lib.mhd_compute_dt(float(cfl), ctypes.byref(dt)))
+        return dt.value
+
+    def step(self, dt):
+        _check(_lib.mhd_step(float(dt)))
+
+    def advance(self, n_steps, cfl, want_time=False):
+        if want_time:
+            t = ctypes.c_double()
+            _check(_lib.mhd_advance(int(n_steps), float(cfl), ctypes.byref(t)))
+            return t.value
+        _check(_lib.mhd_advance(int(n_steps), float(cfl), None))
+        return None
+
+    def max_divb(self):
+        v = ctypes.c_double()
+        _check(_lib.mhd_max_divb(ctypes.byref(v)))
+        return v.value
+
+    def launch_count(self):
+        return int(_lib.mhd_launch_count())
+
+    def synchronize(self):
+        _check(_lib.mhd_synchronize())
+
+    def close(self):
+        _check(_lib.mhd_finalize())
+        self._ws = None

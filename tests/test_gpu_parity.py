@@ -1,0 +1,277 @@
+"""GPU parity: libmhd.so (through the C ABI binding) against the CPU oracle, element by element
+on the same seeded inputs.  Tolerances are BASELINE.json's: max relative difference per field
+<= 1e-12 after one step, <= 1e-9 after a full run, normalised |div B| dx / |B| <= 1e-12 every step.
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_2402_05240_b200 import inputs
+from helpers import run_to_time, divb_normalised, rel_diff, FIELDS, totals
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-12
+TOL_RUN = 1e-9
+TOL_DIVB = 1e-12
+
+
+@pytest.fixture(scope="module")
+def mhd():
+    from paper_2402_05240_b200 import mhd as m
+    return m
+
+
+def make_pair(mhd, p, **kw):
+    o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc)
+    o.set_state(p.state)
+    g = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc, **kw)
+    g.set_state(p.state)
+    return o, g
+
+
+def assert_close(a, b, tol, what):
+    rd = rel_diff(a, b)
+    worst = max(rd.values())
+    assert worst <= tol, "%s: per-field max relative difference %s" % (what, rd)
+    return worst
+
+
+def test_roundtrip_set_get(mhd):
+    p = inputs.random_smooth(n=(37, 21, 19), seed=3)
+    g = mhd.Mhd(*p.n, p.gamma, p.recon)
+    g.set_state(p.state)
+    out = g.get_state()
+    for f in FIELDS:
+        if f in ("bx", "by", "bz"):
+            a = inputs._active(out[f], f)
+            b = inputs._active(p.state[f], f)
+            assert np.array_equal(a, b), f
+        else:
+            assert np.array_equal(out[f], p.state[f]), f
+    g.close()
+
+
+@pytest.mark.parametrize("recon", [0, 1, 2])
+@pytest.mark.parametrize("n", [(37, 21, 19), (130, 9, 34), (16, 70, 5)])
+def test_one_step_random_smooth(mhd, recon, n):
+    """Ragged sizes spanning several x-pencil blocks (127 faces) and march chunks."""
+    p = inputs.random_smooth(n=n, seed=11 + recon, recon=recon)
+    o, g = make_pair(mhd, p)
+    dt_o = o.compute_dt(p.cfl)
+    dt_g = g.compute_dt(p.cfl)
+    assert abs(dt_g - dt_o) <= 1e-13 * dt_o
+    o.step(dt_o)
+    g.step(dt_o)
+    assert_close(g.get_half_state(), o.get_half_state(), TOL_STEP, "half state")
+    out = g.get_state()
+    assert_close(out, o.get_state(), TOL_STEP, "full state")
+    assert divb_normalised(out, p.n) <= TOL_DIVB
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("recon", [1, 2])
+def test_uniform_state_bit_for_bit(mhd, recon):
+    p = inputs.uniform(n=(8, 6, 5), recon=recon)
+    g = mhd.Mhd(*p.n, p.gamma, p.recon)
+    g.set_state(p.state)
+    dt = g.compute_dt(0.4)
+    for _ in range(3):
+        g.step(dt)
+    out = g.get_state()
+    for f in FIELDS:
+        assert np.array_equal(out[f], p.state[f]), f
+    g.close()
+
+
+@pytest.mark.parametrize("n", [(1, 1, 1), (2, 1, 3), (5, 3, 2), (4, 4, 4)])
+@pytest.mark.parametrize("recon", [1, 2])
+def test_tiny_grids(mhd, n, recon):
+    """Grids thinner than the ghost depth: periodic images wrap more than once."""
+    p = inputs.random_smooth(n=(8, 8, 8), seed=5, recon=recon)
+    st = {}
+    sh = inputs.field_shapes(*n)
+    for f in FIELDS:
+        st[f] = np.ascontiguousarray(p.state[f][:sh[f][0], :sh[f][1], :sh[f][2]])
+    # periodic closure of the staggered field: face n equals face 0
+    st["bx"][:, :, -1] = st["bx"][:, :, 0]
+    st["by"][:, -1, :] = st["by"][:, 0, :]
+    st["bz"][-1, :, :] = st["bz"][0, :, :]
+    q = inputs.Problem(name="tiny", n=n, gamma=p.gamma, state=st, recon=recon)
+    o, g = make_pair(mhd, q)
+    dt = o.compute_dt(0.4)
+    assert abs(g.compute_dt(0.4) - dt) <= 1e-13 * dt
+    o.step(dt); g.step(dt)
+    assert_close(g.get_state(), o.get_state(), TOL_STEP, "tiny %s" % (n,))
+    o.close(); g.close()
+
+
+def test_c1_linear_wave_full_run(mhd):
+    """BASELINE.json configs[0]: 32^3 fast wave, one period, vs the oracle and the closed form."""
+    p = inputs.linear_wave(32, 32, 32, "fast", recon=1)
+    o, g = make_pair(mhd, p)
+    n_o = run_to_time(o, p)
+    n_g = run_to_time(g, p)
+    assert n_o == n_g
+    out = g.get_state()
+    assert_close(out, o.get_state(), TOL_RUN, "C1 final state")
+    err = inputs.wave_error(p.state, out)
+    assert err == pytest.approx(6.5165e-8, rel=2e-4)   # tests/golden/linear_wave_errors.txt
+    assert divb_normalised(out, p.n) <= TOL_DIVB
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("axis", [1, 2])
+def test_linear_wave_other_axes_ppmc(mhd, axis):
+    p = inputs.linear_wave(16, 16, 16, "fast", axis=axis, recon=2)
+    o, g = make_pair(mhd, p)
+    run_to_time(o, p); run_to_time(g, p)
+    out = g.get_state()
+    assert_close(out, o.get_state(), TOL_RUN, "PPMC wave axis %d" % axis)
+    assert inputs.wave_error(p.state, out) == pytest.approx(1.189e-7, rel=2e-3)
+    o.close(); g.close()
+
+
+def test_c2_brio_wu_outflow(mhd):
+    """BASELINE.json configs[1]: 256x16x16, outflow in x, to t = 0.1."""
+    p = inputs.riemann("brio_wu", 256, 16, axis=0, recon=1)
+    o, g = make_pair(mhd, p)
+    dt = o.compute_dt(p.cfl)
+    o.step(dt); g.step(dt)
+    assert_close(g.get_state(), o.get_state(), TOL_STEP, "C2 one step")
+    n_o = run_to_time(o, p) + 1
+    t, n_g = dt, 1
+    while t < p.t_end * (1.0 - 1e-14):
+        d = g.compute_dt(p.cfl)
+        if t + d > p.t_end:
+            d = p.t_end - t
+        g.step(d); t += d; n_g += 1
+    out, ref = g.get_state(), o.get_state()
+    # the two runs take their own dt (both from Eq. 11); they must agree to round-off growth
+    assert abs(n_g - n_o) <= 1
+    if n_g == n_o:
+        assert_close(out, ref, 1e-8, "C2 final state")
+    # planar invariants (pin T12)
+    assert np.all(out["bx"] == 0.75)
+    assert np.max(np.abs(out["mz"])) <= 1e-14 and np.max(np.abs(out["bz"])) <= 1e-14
+    assert np.array_equal(out["rho"], np.broadcast_to(out["rho"][0:1, 0:1, :], out["rho"].shape))
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("axis", [1, 2])
+def test_riemann_other_axes_outflow(mhd, axis):
+    p = inputs.riemann("dai_woodward", 64, 8, axis=axis, recon=2, flip=(axis == 2))
+    o, g = make_pair(mhd, p)
+    for _ in range(5):
+        dt = o.compute_dt(p.cfl)
+        o.step(dt); g.step(dt)
+    assert_close(g.get_state(), o.get_state(), 5 * TOL_STEP, "riemann axis %d" % axis)
+    o.close(); g.close()
+
+
+def test_c4_blast_small(mhd):
+    """Shape of BASELINE.json configs[3] at 32^3: PPMC, strong shock, 20 steps; positivity and parity."""
+    p = inputs.blast(32, recon=2, n_steps=20)
+    o, g = make_pair(mhd, p)
+    for s in range(p.n_steps):
+        dt = o.compute_dt(p.cfl)
+        o.step(dt); g.step(dt)
+        if s == 0:
+            assert_close(g.get_state(), o.get_state(), TOL_STEP, "blast step 1")
+    out, ref = g.get_state(), o.get_state()
+    assert_close(out, ref, TOL_RUN, "blast 20 steps")
+    assert np.min(out["rho"]) > 0.0 and np.all(np.isfinite(out["E"]))
+    assert divb_normalised(out, p.n) <= TOL_DIVB
+    o.close(); g.close()
+
+
+def test_c3_turbulence_small_multi_step(mhd):
+    """Shape of BASELINE.json configs[2]/[4] at 48^3: Mach-1 turbulence, beta = 1, PLMC, 5 steps."""
+    p = inputs.turbulence(48, n_steps=5)
+    o, g = make_pair(mhd, p)
+    t0 = totals(p.state)
+    for s in range(p.n_steps):
+        dt = o.compute_dt(p.cfl)
+        assert abs(g.compute_dt(p.cfl) - dt) <= 1e-12 * dt
+        o.step(dt); g.step(dt)
+        out = g.get_state()
+        assert divb_normalised(out, p.n) <= TOL_DIVB
+        assert_close(out, o.get_state(), (s + 1) * 10 * TOL_STEP if s else TOL_STEP, "turbulence step %d" % s)
+    t1 = totals(out)
+    for f in ("rho", "E"):
+        assert abs(t1[f] - t0[f]) <= 1e-13 * abs(t0[f])
+    o.close(); g.close()
+
+
+def test_advance_matches_stepwise_and_device_io(mhd):
+    """mhd_advance (dt kept on the device) == {compute_dt; step} loop; device set/get == host set/get."""
+    import torch
+    p = inputs.random_smooth(n=(40, 24, 18), seed=8, recon=1)
+    g = mhd.Mhd(*p.n, p.gamma, p.recon)
+    g.set_state(p.state)
+    tsum = 0.0
+    for _ in range(3):
+        dt = g.compute_dt(0.4)
+        g.step(dt); tsum += dt
+    ref = g.get_state()
+    dev_in = {f: torch.from_numpy(np.ascontiguousarray(p.state[f])).cuda() for f in FIELDS}
+    g.set_state_device(dev_in)
+    t = g.advance(3, 0.4, want_time=True)
+    assert abs(t - tsum) <= 1e-14 * tsum
+    dev_out = {f: torch.empty_like(dev_in[f]) for f in FIELDS}
+    g.get_state_device(dev_out)
+    torch.cuda.synchronize()
+    for f in FIELDS:
+        assert np.array_equal(dev_out[f].cpu().numpy(), ref[f]), f
+    g.close()
+
+
+def test_internal_cudamalloc_and_stream(mhd):
+    import torch
+    p = inputs.random_smooth(n=(20, 12, 10), seed=9, recon=2)
+    o = orc.Oracle(*p.n, p.gamma, p.recon)
+    o.set_state(p.state)
+    s = torch.cuda.Stream()
+    g = mhd.Mhd(*p.n, p.gamma, p.recon, use_torch_workspace=False, stream=s)
+    g.set_state(p.state)
+    dt = o.compute_dt(0.4)
+    o.step(dt); g.step(dt)
+    assert_close(g.get_state(), o.get_state(), TOL_STEP, "cudaMalloc + stream")
+    g.close(); o.close()
+    mhd.lib().mhd_set_stream(None)
+
+
+def test_error_codes(mhd):
+    L = mhd.lib()
+    L.mhd_finalize()
+    assert L.mhd_step(0.1) == -2
+    assert L.mhd_init(0, 4, 4, 1.4, 1) == -1
+    assert L.mhd_init(4, 4, 4, 1.0, 1) == -1
+    assert L.mhd_init(4, 4, 4, 1.4, 7) == -1
+    assert L.mhd_init(4, 4, 4, 1.4, 1) == 0
+    assert L.mhd_step(-1.0) == -1
+    assert L.mhd_set_boundary(3, 0) == -1
+    # a state with negative pressure is reported by the CFL kernel, not silently floored (G18)
+    p = inputs.uniform(n=(4, 4, 4))
+    st = {k: v.copy() for k, v in p.state.items()}
+    st["E"][1, 2, 3] = 0.0
+    g = mhd.Mhd(4, 4, 4, p.gamma, 1)
+    g.set_state(st)
+    with pytest.raises(mhd.MhdError):
+        g.compute_dt(0.4)
+    g.close()
+
+
+@pytest.mark.timeout(900)
+def test_full_size_256_cube_one_step(mhd):
+    """BASELINE.json configs[2] at full size (256^3, the bench workload and launch configuration):
+    one step against the oracle, every cell."""
+    p = inputs.turbulence(256, n_steps=1)
+    o, g = make_pair(mhd, p)
+    dt = o.compute_dt(p.cfl)
+    assert abs(g.compute_dt(p.cfl) - dt) <= 1e-13 * dt
+    o.step(dt); g.step(dt)
+    out = g.get_state()
+    assert_close(out, o.get_state(), TOL_STEP, "256^3 one step")
+    assert divb_normalised(out, p.n) <= TOL_DIVB
+    o.close(); g.close()
