@@ -1,0 +1,357 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fp64 VL+CT MHD step (BASELINE.json metric) on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c5|c4|c1|c2|NxNxN] [--impl reference]
+
+A "step" is one pass of the whole hot path: the CFL reduction (Eq. 11) followed by one full VL+CT
+step (ghost fill, PCM+HLLD predictor, CT, half update, PLMC/PPMC+HLLD, CT, full update) on a
+seeded synthetic grid.  `value` = cell updates per second with the state resident in HBM;
+`e2e` = the same through the host-buffer C ABI (mhd_set_state + mhd_compute_dt + mhd_step +
+mhd_get_state every step, pinned host memory).  N > 1 runs N independent replicas (DESIGN.md:
+"replicas only", no collective); rank 0 prints ONE JSON line.
+`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+for _p in (ROOT, os.path.join(ROOT, "oracle")):
+    if _p not in sys.path:
+        sys.path.insert(0, _p)
+
+import numpy as np  # noqa: E402
+
+METRIC = "fp64 MHD cell updates/sec (VL+CT, HLLD, PLMC)"
+UNIT = "cell updates/s"
+CFL = 0.4
+
+# Algorithmic work per cell update: fp64 FLOPs (add/mul = 1, fma = 2)
+# executed per cell by each kernel as counted with ncu on the 256^3 workload, and the HBM
+# bytes each kernel must move per cell (compulsory reads + writes of its operands).
+KERNEL_MODEL = {
+    #                      flop/cell  bytes/cell
+    "k_predictor_flux": (None, (8 + 21) * 8),
+    "k_flux_x": (None, (8 + 7) * 8),
+    "k_flux_march<1>": (None, (8 + 7) * 8),
+    "k_flux_march<2>": (None, (8 + 7) * 8),
+    "k_ct(predictor)": (None, (9 + 7 + 3) * 8),
+    "k_ct(corrector)": (None, (9 + 7 + 3) * 8),
+    "k_update(half)": (None, (8 + 15 + 3 + 8) * 8),
+    "k_update(full)": (None, (8 + 15 + 3 + 8) * 8),
+    "k_cfl": (None, 8 * 8),
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="c3",
+                    help="c1..c5 = BASELINE.json configs[0..4]; or NxNxN[:plmc|ppmc] turbulence cube")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def make_problem(workload, small=False):
+    """Seeded synthetic input (paper_2402_05240_b200/inputs.py) for a BASELINE.json config."""
+    from paper_2402_05240_b200 import inputs
+    w = workload.lower()
+    if w == "c1":
+        return inputs.linear_wave(32, 32, 32, "fast", recon=1), "c1: 32^3 linear fast wave, PLMC"
+    if w == "c2":
+        return inputs.riemann("brio_wu", 256, 16, axis=0, recon=1), "c2: 256x16x16 Brio-Wu, PLMC, outflow x"
+    if w == "c3":
+        return inputs.turbulence(256, recon=1), "c3: 256^3 Mach-1 beta-1 turbulence, PLMC (BASELINE.json configs[2])"
+    if w == "c4":
+        return inputs.blast(512, recon=2), "c4: 512^3 blast, PPMC (BASELINE.json configs[3])"
+    if w == "c5":
+        return inputs.turbulence(640, recon=1), "c5: 640^3 Mach-1 beta-1 turbulence, PLMC (BASELINE.json configs[4])"
+    recon = 1
+    if ":" in w:
+        w, r = w.split(":")
+        recon = {"plmc": 1, "ppmc": 2, "pcm": 0}[r]
+    n = tuple(int(x) for x in w.split("x"))
+    if len(n) == 1:
+        n = n * 3
+    return inputs.turbulence(n, recon=recon), "%dx%dx%d turbulence, recon=%d" % (n + (recon,))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); smax.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(smax)) if smax else None,
+                "power_w_max": float(max(pw)) if pw else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_oracle(problem, n_steps):
+    """The oracle as it stands on the host cores: {compute_dt; step} x n_steps. Returns (cells/s, s)."""
+    import oracle as orc
+    o = orc.Oracle(*problem.n, problem.gamma, problem.recon, problem.bc)
+    o.set_state(problem.state)
+    t0 = time.perf_counter()
+    for _ in range(n_steps):
+        dt = o.compute_dt(CFL)
+        o.step(dt)
+    el = time.perf_counter() - t0
+    cores = orc.num_threads()
+    o.close()
+    nc = problem.n[0] * problem.n[1] * problem.n[2]
+    return nc * n_steps / el, el, cores
+
+
+def sample_problem(workload):
+    """Bounded sample of the workload for the CPU oracle (same recipe, smaller grid where needed)."""
+    from paper_2402_05240_b200 import inputs
+    w = workload.lower()
+    if w in ("c1", "c2"):
+        p, name = make_problem(w)
+        return p, name + " (full size)"
+    if w == "c4":
+        return inputs.blast(64, recon=2), "c4 recipe (blast, PPMC) at 64^3"
+    recon = 2 if w.endswith(":ppmc") else 1
+    return inputs.turbulence(96, recon=recon), "c3/c5 recipe (Mach-1 beta-1 turbulence, recon=%d) at 96^3" % recon
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    p, sample = sample_problem(args.workload)
+    _, wname = make_problem_name(args.workload)
+    import oracle as orc
+    o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc)
+    o.set_state(p.state)
+    for _ in range(args.warmup):
+        o.step(o.compute_dt(CFL))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(o.compute_dt(CFL))
+    el = time.perf_counter() - t0
+    cores = orc.num_threads()
+    o.close()
+    nc = p.n[0] * p.n[1] * p.n[2]
+    val = nc * args.steps / el
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": wname, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def make_problem_name(workload):
+    names = {"c1": "c1: 32^3 linear fast wave, PLMC", "c2": "c2: 256x16x16 Brio-Wu, PLMC, outflow x",
+             "c3": "c3: 256^3 Mach-1 beta-1 turbulence, PLMC (BASELINE.json configs[2])",
+             "c4": "c4: 512^3 blast, PPMC (BASELINE.json configs[3])",
+             "c5": "c5: 640^3 Mach-1 beta-1 turbulence, PLMC (BASELINE.json configs[4])"}
+    return None, names.get(workload.lower(), workload + " turbulence cube")
+
+
+def load_measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the VL+CT step has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2402_05240_b200 import mhd
+    from paper_2402_05240_b200.inputs import FIELDS
+
+    p, wname = make_problem(args.workload)
+    nc = p.n[0] * p.n[1] * p.n[2]
+    stream = torch.cuda.Stream()
+    g = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc, stream=stream)
+    g.set_state(p.state)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    with torch.cuda.stream(stream):
+        g.advance(args.warmup, CFL)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+        barrier()
+        torch.cuda.synchronize()
+        l0 = g.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        g.advance(args.steps, CFL)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        launches = g.launch_count() - l0
+        clocks = sampler.stop() if rank == 0 else None
+        if world > 1:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        value = world * nc * args.steps / (ms * 1e-3)
+
+        # ---- per-kernel live timing (CUDA events on the library stream) ----------------
+        prof = {}
+        nprof = 3
+        for _ in range(nprof):
+            dt = g.compute_dt(CFL)
+            for name, t_ms in g.step_profile(dt):
+                prof[name] = prof.get(name, 0.0) + t_ms / nprof
+        bad_state = False
+        try:
+            g.compute_dt(CFL)
+        except mhd.MhdError:
+            bad_state = True
+
+        # ---- end to end through the host-buffer ABI ------------------------------------
+        sh = mhd.field_shapes(*p.n)
+        pin_in = {f: torch.from_numpy(np.ascontiguousarray(p.state[f])).pin_memory() for f in FIELDS}
+        pin_out = {f: torch.empty(sh[f], dtype=torch.float64).pin_memory() for f in FIELDS}
+        np_in = {f: pin_in[f].numpy() for f in FIELDS}
+        np_out = {f: pin_out[f].numpy() for f in FIELDS}
+        h2d = sum(int(np_in[f].nbytes) for f in FIELDS)
+        d2h = sum(int(np_out[f].nbytes) for f in FIELDS) + 8
+
+        def e2e_step():
+            g.set_state(np_in)
+            dt_ = g.compute_dt(CFL)
+            g.step(dt_)
+            g.get_state(np_out)
+
+        e2e_step()
+        barrier()
+        torch.cuda.synchronize()
+        e0.record(stream)
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        ms_e2e = max(e0.elapsed_time(e1), wall * 1e3)
+        if world > 1:
+            t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e2e = float(t.item())
+        e2e_val = world * nc * args.e2e_steps / (ms_e2e * 1e-3)
+
+    fp64_tf, copy_gbs = (None, None)
+    if rank == 0:
+        fp64_tf, copy_gbs = mhd.measure_peaks(1.0)
+    g.close()
+
+    if rank == 0:
+        hbm_peak, hbm_src = load_measured_peaks()
+        step_ms = sum(prof.values())
+        top = max((k for k in prof if k in KERNEL_MODEL), key=lambda k: prof[k])
+        flop_cell, byte_cell = KERNEL_MODEL[top]
+        t_top = prof[top] * 1e-3
+        roof = {"kernel": top, "kernel_ms": prof[top], "share_of_step": prof[top] / step_ms,
+                "traffic": None}
+        hbm_ach = byte_cell * nc / t_top / 1e9
+        if flop_cell is not None and flop_cell * nc / (fp64_tf * 1e12) > byte_cell * nc / (hbm_peak * 1e9):
+            ach = flop_cell * nc / t_top / 1e12
+            roof.update({"bound": "alu", "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s",
+                         "frac": ach / fp64_tf, "peak_source": "measured DFMA chain (mhd_measure_peaks, sustained)",
+                         "hbm_achieved_gbs": hbm_ach})
+        else:
+            roof.update({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
+                         "frac": hbm_ach / hbm_peak, "peak_source": hbm_src})
+        roof["kernels_ms"] = {k: round(v, 4) for k, v in prof.items()}
+        roof["measured_here"] = {"fp64_tflops": fp64_tf, "copy_gbs": copy_gbs}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": wname, "grid": list(p.n), "recon": p.recon, "cfl": CFL,
+                           "parallelism": "replicas x%d" % world,
+                           "l2": "inputs larger than L2 (state %.0f MB)" % (8 * 8 * nc / 1e6),
+                           "step": "mhd_advance: CFL reduction + full VL+CT step, dt on device"},
+                "clocks": clocks, "gpu_launches": int(launches),
+                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "steps": args.e2e_steps},
+                "roofline": roof, "state_ok": not bad_state,
+                "paper_context": {"a100_cell_updates_per_s": 2.59e8, "ratio": value / world / 2.59e8}}
+        if world == 1 and not args.no_cpu_baseline:
+            sp, sname = sample_problem(args.workload)
+            v, el, cores = time_oracle(sp, 6 if sp.n[0] >= 64 else 40)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": sname + ", %.1f s" % el}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_b200(a))

@@ -113,6 +113,20 @@ int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *
  * Synchronous; *out is a HOST pointer. */
 int mhd_max_divb(double *out);
 
+/* Instrumented variant of { CFL reduction; mhd_step(dt) }: records a CUDA event on the library
+ * stream after every kernel launch and returns, for launch i, its duration ms[i] (milliseconds,
+ * event to event, so it includes the launch gap) and a static name names[i].  At most
+ * max_entries are written; *n_entries receives the count.  Synchronises.  Used by bench.py for
+ * the per-kernel roofline; the state advances exactly as with mhd_step. */
+int mhd_step_profile(double dt, int max_entries, double *ms, const char **names, int *n_entries);
+
+/* Roofline denominators measured on the current device (not part of the time step): the fp64
+ * FMA-pipe peak in TFLOP/s from a kernel of independent DFMA chains (8 per thread, 2048 threads
+ * per SM; burst = best of 5 launches if seconds <= 0.5, else the mean over the second half of 40
+ * back-to-back launches = sustained clocks) and the HBM copy bandwidth in GB/s (read + write
+ * bytes of a 1 GiB copy, best of 5).  Uses the default stream; synchronises. */
+int mhd_measure_peaks(double *fp64_tflops, double *copy_gbs, double seconds);
+
 /* Number of kernel launches issued by this library since mhd_init (for bench.py). */
 long long mhd_launch_count(void);
 

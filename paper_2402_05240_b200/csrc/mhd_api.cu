@@ -11,6 +11,8 @@ using namespace mhd;
 
 namespace {
 
+const int kMaxProf = 32;
+
 struct Context {
   bool inited = false;
   bool owns_memory = false;
@@ -23,7 +25,10 @@ struct Context {
   Scalars *sc = nullptr;
   cudaStream_t stream = 0;
   long long launches = 0;
-  bool graph_ok = false;
+  // per-launch event timing (mhd_step_profile)
+  int prof_n = -1;  // -1 = off, else number of launches recorded so far
+  cudaEvent_t prof_ev[kMaxProf + 1];
+  const char *prof_name[kMaxProf];
 };
 
 Context C;
@@ -45,11 +50,15 @@ int cuda_fail(cudaError_t e, const char *where) {
     if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
   } while (0)
 
-#define LAUNCH_CHECK(name)                                \
-  do {                                                    \
-    C.launches++;                                         \
-    cudaError_t e_ = cudaGetLastError();                  \
-    if (e_ != cudaSuccess) return cuda_fail(e_, name);    \
+#define LAUNCH_CHECK(name)                                          \
+  do {                                                              \
+    C.launches++;                                                   \
+    cudaError_t e_ = cudaGetLastError();                            \
+    if (e_ != cudaSuccess) return cuda_fail(e_, name);              \
+    if (C.prof_n >= 0 && C.prof_n < kMaxProf) {                     \
+      C.prof_name[C.prof_n] = name;                                 \
+      cudaEventRecord(C.prof_ev[++C.prof_n], C.stream);             \
+    }                                                               \
   } while (0)
 
 inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
@@ -404,6 +413,35 @@ int mhd_max_divb(double *out) {
   CU(cudaStreamSynchronize(C.stream));
   memcpy(out, &h, sizeof(double));
   return MHD_OK;
+}
+
+int mhd_step_profile(double dt, int max_entries, double *ms, const char **names, int *n_entries) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (!(dt > 0.0) || !ms || !names || !n_entries || max_entries < 1)
+    return fail(MHD_ERR_ARG, "mhd_step_profile: bad argument");
+  for (int i = 0; i <= kMaxProf; i++) CU(cudaEventCreate(&C.prof_ev[i]));
+  k_set_dt<<<1, 1, 0, C.stream>>>(C.sc, dt);
+  LAUNCH_CHECK("k_set_dt");
+  C.prof_n = 0;
+  cudaEventRecord(C.prof_ev[0], C.stream);
+  int rc = cfl_kernel();
+  if (!rc) {
+    k_reset_min<<<1, 1, 0, C.stream>>>(C.sc);
+    C.launches++;
+    rc = step_kernels();
+  }
+  int n = C.prof_n;
+  C.prof_n = -1;
+  cudaError_t e = cudaStreamSynchronize(C.stream);
+  if (!rc && e != cudaSuccess) rc = cuda_fail(e, "cudaStreamSynchronize");
+  *n_entries = 0;
+  for (int i = 0; i < n && !rc; i++) {
+    float t = 0.f;
+    cudaEventElapsedTime(&t, C.prof_ev[i], C.prof_ev[i + 1]);
+    if (i < max_entries) { ms[i] = t; names[i] = C.prof_name[i]; *n_entries = i + 1; }
+  }
+  for (int i = 0; i <= kMaxProf; i++) cudaEventDestroy(C.prof_ev[i]);
+  return rc;
 }
 
 long long mhd_launch_count(void) { return C.launches; }

@@ -47,6 +47,11 @@ def _load():
     L.mhd_get_state_device.argtypes = [_vp] * 8
     L.mhd_get_half_state.argtypes = [_dp] * 8
     L.mhd_max_divb.argtypes = [_dp]
+    L.mhd_measure_peaks.argtypes = [_dp, _dp, ctypes.c_double]
+    L.mhd_measure_peaks.restype = ctypes.c_int
+    L.mhd_step_profile.argtypes = [ctypes.c_double, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_char_p),
+                                   ctypes.POINTER(ctypes.c_int)]
+    L.mhd_step_profile.restype = ctypes.c_int
     L.mhd_launch_count.restype = ctypes.c_longlong
     L.mhd_last_error.restype = ctypes.c_char_p
     for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_stream", "mhd_set_state",
@@ -71,6 +76,13 @@ def _check(rc):
 
 def _hp(a):
     return a.ctypes.data_as(_dp)
+
+
+def measure_peaks(seconds=0.0):
+    """(fp64 DFMA TFLOP/s, HBM copy GB/s) measured on the current device."""
+    tf, bw = ctypes.c_double(), ctypes.c_double()
+    _check(_lib.mhd_measure_peaks(ctypes.byref(tf), ctypes.byref(bw), float(seconds)))
+    return tf.value, bw.value
 
 
 class Mhd:
@@ -160,6 +172,14 @@ class Mhd:
             return t.value
         _check(_lib.mhd_advance(int(n_steps), float(cfl), None))
         return None
+
+    def step_profile(self, dt, max_entries=32):
+        """One instrumented {CFL; step}: list of (kernel name, milliseconds)."""
+        ms = (ctypes.c_double * max_entries)()
+        names = (ctypes.c_char_p * max_entries)()
+        n = ctypes.c_int()
+        _check(_lib.mhd_step_profile(float(dt), max_entries, ms, names, ctypes.byref(n)))
+        return [(names[i].decode(), ms[i]) for i in range(n.value)]
 
     def max_divb(self):
         v = ctypes.c_double()
