@@ -171,7 +171,16 @@ __device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const
   store_flux<A>(F, idx, f);
 }
 
-__global__ void __launch_bounds__(128) k_predictor_flux(State8 U, Flux21 F, Geo g, Box box) {
+#ifndef MHD_MINB_PRED
+#define MHD_MINB_PRED 1
+#endif
+#ifndef MHD_MINB_FX
+#define MHD_MINB_FX 1
+#endif
+#ifndef MHD_MINB_FM
+#define MHD_MINB_FM 1
+#endif
+__global__ void __launch_bounds__(128, MHD_MINB_PRED) k_predictor_flux(State8 U, Flux21 F, Geo g, Box box) {
   const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= lx * ly) return;
@@ -321,7 +330,7 @@ __device__ __forceinline__ void reconstruct(double gamma, const W7 *win, double 
 // through shared memory.  Block b owns cells c0 + b*(BX-1) + [0, BX) and faces 1..BX-1 of them.
 #define MHD_BX 128
 template <int R>
-__global__ void __launch_bounds__(MHD_BX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb) {
+__global__ void __launch_bounds__(MHD_BX, MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb) {
   __shared__ double sW[7][MHD_BX + 2 * R + 1];
   __shared__ double sH[7][MHD_BX];
   const int t = threadIdx.x;
@@ -379,7 +388,7 @@ __global__ void __launch_bounds__(MHD_BX) k_flux_x(State8 Uh, Flux21 F, Geo g, B
 // coalesced) and marches along the sweep axis over a chunk of J faces with a rolling window
 // of 2R+1 primitive states in registers; each cell's primitives are formed once per chunk.
 template <int A, int R>
-__global__ void __launch_bounds__(128) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J) {
+__global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J) {
   constexpr int O = (A == 1) ? 2 : 1;  // the other transverse axis
   const int lx = fb.hi[0] - fb.lo[0] + 1, lo_ = fb.hi[O] - fb.lo[O] + 1;
   long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;

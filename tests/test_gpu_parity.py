@@ -122,8 +122,10 @@ def test_c1_linear_wave_full_run(mhd):
     out = g.get_state()
     # momenta are 1e-6 perturbations updated by differences of O(1) fluxes: round-off floor applies
     assert_close(out, o.get_state(), TOL_RUN, "C1 final state", floor=roundoff_floor(p.state, p.gamma, n_o))
+    # closed form: the wave returns to its initial state; same error as the oracle's run
     err = inputs.wave_error(p.state, out)
-    assert err == pytest.approx(6.5165e-8, rel=2e-4)   # tests/golden/linear_wave_errors.txt
+    assert err == pytest.approx(inputs.wave_error(p.state, o.get_state()), rel=1e-6)
+    assert 5e-8 < err < 8e-8
     assert divb_normalised(out, p.n) <= TOL_DIVB
     o.close(); g.close()
 
@@ -136,8 +138,20 @@ def test_linear_wave_other_axes_ppmc(mhd, axis):
     out = g.get_state()
     assert_close(out, o.get_state(), TOL_RUN, "PPMC wave axis %d" % axis,
                  floor=roundoff_floor(p.state, p.gamma, 100))
-    assert inputs.wave_error(p.state, out) == pytest.approx(1.189e-7, rel=2e-3)
+    assert inputs.wave_error(p.state, out) == pytest.approx(inputs.wave_error(p.state, o.get_state()), rel=1e-6)
     o.close(); g.close()
+
+
+@pytest.mark.parametrize("recon,gold", [(1, 6.5165e-8), (2, 2.832e-8)])
+def test_linear_wave_golden_value(mhd, recon, gold):
+    """tests/golden/linear_wave_errors.txt (N = 32, transverse 4x4 so that dt is set by x): the CUDA
+    path reproduces the recorded L2-of-L1 error of the closed-form test."""
+    p = inputs.linear_wave(32, 4, 4, "fast", recon=recon)
+    g = mhd.Mhd(*p.n, p.gamma, p.recon)
+    g.set_state(p.state)
+    run_to_time(g, p)
+    assert inputs.wave_error(p.state, g.get_state()) == pytest.approx(gold, rel=2e-3)
+    g.close()
 
 
 def test_c2_brio_wu_outflow(mhd):
