@@ -109,6 +109,12 @@ int mhd_get_state_device(double *rho, double *mx, double *my, double *mz, double
 int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *E, double *bx,
                        double *by, double *bz);
 
+/* Debug/parity: component comp (0 mass, 1 mom_n, 2 mom_t1, 3 mom_t2, 4 energy, 5 B_t1 flux,
+ * 6 B_t2 flux; solver-local axes of reading O0) of the corrector HLLD flux on
+ * the LOWER `axis`-face of every active cell, as left by the last mhd_step; nx*ny*nz values to a
+ * HOST array.  Overwrites the stored half-step state.  Synchronises. */
+int mhd_get_flux(int axis, int comp, double *out);
+
 /* max over active cells of |sum_a (B_a[upper] - B_a[lower]) / Delta_a|.
  * Synchronous; *out is a HOST pointer. */
 int mhd_max_divb(double *out);
@@ -126,6 +132,29 @@ int mhd_step_profile(double dt, int max_entries, double *ms, const char **names,
  * back-to-back launches = sustained clocks) and the HBM copy bandwidth in GB/s (read + write
  * bytes of a 1 GiB copy, best of 5).  Uses the default stream; synchronises. */
 int mhd_measure_peaks(double *fp64_tflops, double *copy_gbs, double seconds);
+
+/* Unit-level entry points (tests compare the device arithmetic with the oracle function by
+ * function).  All pointers are HOST pointers; the calls are synchronous on the default stream and
+ * need no context.  Solver-local 1-D states W = (rho, u, v, w, P, B_t1, B_t2) (reading O0).
+ *
+ * mhd_unit_hlld: n independent HLLD solves (reading O4): WL, WR are n*7 values,
+ * bx n face-normal fields, F receives n*7 flux components (mass, mom_n, mom_t1, mom_t2, energy,
+ * B_t1 flux, B_t2 flux). */
+int mhd_unit_hlld(int n, double gamma, const double *WL, const double *WR, const double *bx,
+                  double *F);
+
+/* n independent reconstructions of one cell: recon = MHD_RECON_PLMC (Eq. 23-28, PAPER.md:229-263;
+ * stencil of 3 states) or MHD_RECON_PPMC (reading O10; stencil of 5 states).  Ws holds
+ * n * (2*recon+1) * 7 values (stencil cell fastest after the component), bn0 the n cell-centred
+ * normal fields of the middle cell.  Wlo = W_{R,i-1/2}, Whi = W_{L,i+1/2}, n*7 values each. */
+int mhd_unit_reconstruct(int n, double gamma, int recon, const double *Ws, const double *bn0,
+                         double *Wlo, double *Whi);
+
+/* n independent CT edge fields (Eq. 15-18, reading O6).  in12 holds, per edge,
+ * (Ea0, Ea1, Eb0, Eb1, Ma0, Ma1, Mb0, Mb1, Er00, Er10, Er01, Er11) as named in reading O6:
+ * face fields on the two a-faces and two b-faces touching the edge, the mass fluxes on those
+ * faces, and the reference field of the four cells around the edge. */
+int mhd_unit_ct_edge(int n, const double *in12, double *out);
 
 /* Number of kernel launches issued by this library since mhd_init (for bench.py). */
 long long mhd_launch_count(void);

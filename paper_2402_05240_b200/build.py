@@ -10,7 +10,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmhd.so")
-SOURCES = [os.path.join(CSRC, "mhd_api.cu"), os.path.join(CSRC, "mhd_peaks.cu")]
+SOURCES = [os.path.join(CSRC, "mhd_api.cu"), os.path.join(CSRC, "mhd_peaks.cu"),
+           os.path.join(CSRC, "mhd_unit.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mhd_device.cuh", "mhd_grid.cuh", "mhd_kernels.cuh")] + [
     os.path.join(ROOT, "include", "mhd.h")]
 

@@ -127,6 +127,9 @@ int launch_corrector_fluxes() {
   {
     Box fb = make_box(-1, n0, 0, n1, -1, n2);
     int J = (n1 + 1 >= 64) ? 32 : ((n1 + 1 >= 16) ? 8 : 4);
+#ifdef MHD_FORCE_J
+    J = MHD_FORCE_J;
+#endif
     long long nt = (long long)(n0 + 2) * (n2 + 2);
     dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
     k_flux_march<1, R><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J);
@@ -394,6 +397,19 @@ int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *
   double *dst[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
   int rc = get_state_to(C.Uh, dst, true);
   if (rc) return rc;
+  CU(cudaStreamSynchronize(C.stream));
+  return MHD_OK;
+}
+
+int mhd_get_flux(int axis, int comp, double *out) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (axis < 0 || axis > 2 || comp < 0 || comp > 6 || !out) return fail(MHD_ERR_ARG, "mhd_get_flux: bad argument");
+  const Geo &g = C.g;
+  long long cnt = (long long)g.n[0] * g.n[1] * g.n[2];
+  double *stage = C.Uh.f[0];  // the half-step state is dead after the step
+  k_pack<<<grid1(cnt, 256), 256, 0, C.stream>>>(stage, C.F.f[axis][comp], g, g.n[0], g.n[1], g.n[2]);
+  LAUNCH_CHECK("k_pack");
+  CU(cudaMemcpyAsync(out, stage, cnt * sizeof(double), cudaMemcpyDeviceToHost, C.stream));
   CU(cudaStreamSynchronize(C.stream));
   return MHD_OK;
 }

@@ -151,6 +151,9 @@ __device__ __forceinline__ F7 hlld(double gamma, const W7 &WL, const W7 &WR, dou
     F.bz += Ss * (bzss - a.bzs);
     // mass and normal momentum: U** - U* = 0 exactly
   }
+  // reading R6: a contact slower than 1e-13 of the fast speed is at rest -- the mass flux, whose
+  // sign upwinds the CT terms (Eq. 16, G6), is then exactly zero ("otherwise" branch: average)
+  if (fabs(F.m) <= 1e-13 * (L.rho + R.rho) * cfmax) F.m = 0.0;
   return F;
 }
 
@@ -205,45 +208,50 @@ __device__ __forceinline__ void eig_setup(Eig &e, double gamma, const W7 &W, dou
   e.Ssr = S * sr; e.Sisr = S / sr;
 }
 
-// a = L . x   (x in the component order of W7)
+// a = L . x   (x in the component order of W7).  Written with explicit rounding intrinsics so
+// that every inlined copy is the same instruction sequence: PPMC projects the five stencil
+// states separately, and the limiter's tests (reading O10: "<= 0" includes equality) must see
+// bit-identical amplitudes for bit-identical states (an exact plateau next to a jump).
 __device__ __forceinline__ C7 eig_left(const Eig &e, const W7 &x) {
-  double xp = e.betay * x.v + e.betaz * x.w;
-  double xq = e.betay * x.w - e.betaz * x.v;
-  double bp = e.betay * x.by + e.betaz * x.bz;
-  double bq = e.betay * x.bz - e.betaz * x.by;
-  double f1 = e.Cff * x.u - e.Qs * xp;
-  double f2 = (e.alf * x.P + e.As * bp) * e.irho;
-  double s1 = e.Css * x.u + e.Qf * xp;
-  double s2 = (e.als * x.P - e.Af * bp) * e.irho;
-  double q2 = e.Sisr * bq;
+  double xp = __fma_rn(e.betay, x.v, __dmul_rn(e.betaz, x.w));
+  double xq = __fma_rn(e.betay, x.w, -__dmul_rn(e.betaz, x.v));
+  double bp = __fma_rn(e.betay, x.by, __dmul_rn(e.betaz, x.bz));
+  double bq = __fma_rn(e.betay, x.bz, -__dmul_rn(e.betaz, x.by));
+  double f1 = __fma_rn(e.Cff, x.u, -__dmul_rn(e.Qs, xp));
+  double f2 = __dmul_rn(__fma_rn(e.alf, x.P, __dmul_rn(e.As, bp)), e.irho);
+  double s1 = __fma_rn(e.Css, x.u, __dmul_rn(e.Qf, xp));
+  double s2 = __dmul_rn(__fma_rn(e.als, x.P, -__dmul_rn(e.Af, bp)), e.irho);
+  double q2 = __dmul_rn(e.Sisr, bq);
   C7 c;
-  c.c0 = e.N * (f2 - f1);
-  c.c6 = e.N * (f2 + f1);
-  c.c2 = e.N * (s2 - s1);
-  c.c4 = e.N * (s2 + s1);
-  c.c1 = 0.5 * (q2 + xq);
-  c.c5 = 0.5 * (q2 - xq);
-  c.c3 = x.rho - x.P * e.ia2;
+  c.c0 = __dmul_rn(e.N, __dadd_rn(f2, -f1));
+  c.c6 = __dmul_rn(e.N, __dadd_rn(f2, f1));
+  c.c2 = __dmul_rn(e.N, __dadd_rn(s2, -s1));
+  c.c4 = __dmul_rn(e.N, __dadd_rn(s2, s1));
+  c.c1 = __dmul_rn(0.5, __dadd_rn(q2, xq));
+  c.c5 = __dmul_rn(0.5, __dadd_rn(q2, -xq));
+  c.c3 = __fma_rn(-x.P, e.ia2, x.rho);
   return c;
 }
 
-// x = R . a
+// x = R . a   (explicit roundings for the same reason: the two faces of a cell whose limited
+// amplitudes are bit-identical must get bit-identical states, so that a face between mirror-image
+// cells at rest sees W_L == W_R and an exactly zero mass flux -- the "average" branch of Eq. 16)
 __device__ __forceinline__ W7 eig_right(const Eig &e, const C7 &c) {
-  double fs = c.c0 + c.c6, fd = c.c6 - c.c0;
-  double ss = c.c2 + c.c4, sd = c.c4 - c.c2;
-  double as_ = c.c1 + c.c5, ad = c.c1 - c.c5;
-  double comp = e.alf * fs + e.als * ss;
-  double tp = e.Qf * sd - e.Qs * fd;   // transverse velocity along B_perp
-  double bp = e.As * fs - e.Af * ss;   // transverse field along B_perp
-  double bq = e.Ssr * as_;             // transverse field across B_perp
+  double fs = __dadd_rn(c.c0, c.c6), fd = __dadd_rn(c.c6, -c.c0);
+  double ss = __dadd_rn(c.c2, c.c4), sd = __dadd_rn(c.c4, -c.c2);
+  double as_ = __dadd_rn(c.c1, c.c5), ad = __dadd_rn(c.c1, -c.c5);
+  double comp = __fma_rn(e.alf, fs, __dmul_rn(e.als, ss));
+  double tp = __fma_rn(e.Qf, sd, -__dmul_rn(e.Qs, fd));   // transverse velocity along B_perp
+  double bp = __fma_rn(e.As, fs, -__dmul_rn(e.Af, ss));   // transverse field along B_perp
+  double bq = __dmul_rn(e.Ssr, as_);                      // transverse field across B_perp
   W7 x;
-  x.rho = e.rho * comp + c.c3;
-  x.u = e.Cff * fd + e.Css * sd;
-  x.v = e.betay * tp - e.betaz * ad;
-  x.w = e.betaz * tp + e.betay * ad;
-  x.P = e.rho * e.a2 * comp;
-  x.by = e.betay * bp - e.betaz * bq;
-  x.bz = e.betaz * bp + e.betay * bq;
+  x.rho = __fma_rn(e.rho, comp, c.c3);
+  x.u = __fma_rn(e.Cff, fd, __dmul_rn(e.Css, sd));
+  x.v = __fma_rn(e.betay, tp, -__dmul_rn(e.betaz, ad));
+  x.w = __fma_rn(e.betaz, tp, __dmul_rn(e.betay, ad));
+  x.P = __dmul_rn(__dmul_rn(e.rho, e.a2), comp);
+  x.by = __fma_rn(e.betay, bp, -__dmul_rn(e.betaz, bq));
+  x.bz = __fma_rn(e.betaz, bp, __dmul_rn(e.betay, bq));
   return x;
 }
 
@@ -315,8 +323,14 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
   double qm = ppm_face(q0, q1, q2, q3);
   double qp = ppm_face(q1, q2, q3, q4);
   double qi = q2;
-  double dm = qi - qm, dp = qp - qi;
-  if (dm * dp <= 0.0 || (q3 - qi) * (qi - q1) <= 0.0) {
+  // reading R7: differences that are zero to round-off count as zero in the extremum test
+  double tau = 1e-12 * fmax(fabs(q1), fmax(fabs(q2), fabs(q3)));
+  double dm = qi - qm, dp = qp - qi, e3 = q3 - qi, e1 = qi - q1;
+  dm = (fabs(dm) <= tau) ? 0.0 : dm;
+  dp = (fabs(dp) <= tau) ? 0.0 : dp;
+  e3 = (fabs(e3) <= tau) ? 0.0 : e3;
+  e1 = (fabs(e1) <= tau) ? 0.0 : e1;
+  if (dm * dp <= 0.0 || e3 * e1 <= 0.0) {
     double Df = 6.0 * (qm - 2.0 * qi + qp);
     double Dm1 = q0 - 2.0 * q1 + q2;
     double D0 = q1 - 2.0 * q2 + q3;
@@ -325,7 +339,7 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
     double s = sgn3(Df);
     if (s != 0.0 && s == sgn3(Dm1) && s == sgn3(D0) && s == sgn3(Dp1))
       Dlim = s * fmin(fmin(C * fabs(Dm1), C * fabs(D0)), fmin(C * fabs(Dp1), fabs(Df)));
-    if (fabs(Df) > 1e-12 * fmax(fabs(q1), fmax(fabs(q2), fabs(q3)))) r = Dlim / Df;
+    if (fabs(Df) > tau) r = Dlim / Df;
     if (r <= 1.0 - 1e-12) { qm = qi - r * dm; qp = qi + r * dp; }
   } else {
     if (fabs(dm) >= 2.0 * fabs(dp)) qm = qi - 2.0 * dp;

@@ -64,8 +64,12 @@ __device__ __forceinline__ Prim load_prim(const State8 &U, const Geo &g, long lo
     p.v[a] = __ldg(U.f[F_MX + a] + idx) * ir;
   }
   double E = __ldg(U.f[F_E] + idx);
-  p.P = (g.gamma - 1.0) * (E - 0.5 * rho * (p.v[0] * p.v[0] + p.v[1] * p.v[1] + p.v[2] * p.v[2]) -
-                           0.5 * (p.B[0] * p.B[0] + p.B[1] * p.B[1] + p.B[2] * p.B[2]));
+  // explicit roundings: every inlined copy is the same instruction sequence, so bit-identical
+  // cells give bit-identical primitives (the limiters' "<= 0" tests include equality, O10)
+  double v2 = __fma_rn(p.v[2], p.v[2], __fma_rn(p.v[1], p.v[1], __dmul_rn(p.v[0], p.v[0])));
+  double b2 = __fma_rn(p.B[2], p.B[2], __fma_rn(p.B[1], p.B[1], __dmul_rn(p.B[0], p.B[0])));
+  double ek = __dmul_rn(__dmul_rn(0.5, rho), v2);
+  p.P = __dmul_rn(g.gamma - 1.0, __fma_rn(-0.5, b2, __dadd_rn(E, -ek)));
   return p;
 }
 

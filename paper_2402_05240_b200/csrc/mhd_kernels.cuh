@@ -400,15 +400,19 @@ __global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux
   long long idx = (A == 1) ? cell_index(g, i, f0, o) : cell_index(g, i, o, f0);  // cell f0
   W7 win[2 * R + 1];
   double bnc[2 * R + 1];
-  // window centred on cell f0-1
+  // window centred on cell f0-2 (slot 0 is never used): the loop below first shifts it
 #pragma unroll
-  for (int s = 0; s < 2 * R + 1; s++) {
-    Prim p = load_prim(Uh, g, idx + (long long)(s - R - 1) * sA);
+  for (int s = 1; s < 2 * R + 1; s++) {
+    Prim p = load_prim(Uh, g, idx + (long long)(s - R - 2) * sA);
     win[s] = to_W<A>(p, bnc[s]);
   }
-  W7 WL, lo, hi;
-  reconstruct<R>(g.gamma, win, bnc[R], lo, WL);
-  for (int f = f0; f <= f1; f++, idx += sA) {
+  win[0] = win[1]; bnc[0] = bnc[1];
+  W7 WL = win[1], lo, hi;
+  idx -= sA;
+  // One reconstruct() call site per kernel: iteration f0-1 only produces W_L of face f0; every
+  // cell is then reconstructed by the same instruction sequence, so mirror-image cells give
+  // mirror-image states bit for bit.
+  for (int f = f0 - 1; f <= f1; f++, idx += sA) {
 #pragma unroll
     for (int s = 0; s < 2 * R; s++) { win[s] = win[s + 1]; bnc[s] = bnc[s + 1]; }
     {
@@ -416,8 +420,10 @@ __global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux
       win[2 * R] = to_W<A>(p, bnc[2 * R]);
     }
     reconstruct<R>(g.gamma, win, bnc[R], lo, hi);
-    F7 fl = hlld(g.gamma, WL, lo, __ldg(Uh.f[F_BX + A] + idx));
-    store_flux<A>(F, idx, fl);
+    if (f >= f0) {
+      F7 fl = hlld(g.gamma, WL, lo, __ldg(Uh.f[F_BX + A] + idx));
+      store_flux<A>(F, idx, fl);
+    }
     WL = hi;
   }
 }

@@ -13,7 +13,8 @@ import numpy as np
 from .inputs import FIELDS, field_shapes
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmhd.so")
+# MHD_LIBRARY overrides the in-tree build (e.g. to compare two builds of the same ABI)
+LIB_PATH = os.environ.get("MHD_LIBRARY") or os.path.join(_HERE, "libmhd.so")
 
 RECON_PCM, RECON_PLMC, RECON_PPMC = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW = 0, 1
@@ -47,17 +48,21 @@ def _load():
     L.mhd_get_state_device.argtypes = [_vp] * 8
     L.mhd_get_half_state.argtypes = [_dp] * 8
     L.mhd_max_divb.argtypes = [_dp]
+    L.mhd_get_flux.argtypes = [ctypes.c_int, ctypes.c_int, _dp]
     L.mhd_measure_peaks.argtypes = [_dp, _dp, ctypes.c_double]
     L.mhd_measure_peaks.restype = ctypes.c_int
     L.mhd_step_profile.argtypes = [ctypes.c_double, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_char_p),
                                    ctypes.POINTER(ctypes.c_int)]
     L.mhd_step_profile.restype = ctypes.c_int
+    L.mhd_unit_hlld.argtypes = [ctypes.c_int, ctypes.c_double, _dp, _dp, _dp, _dp]
+    L.mhd_unit_reconstruct.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_int, _dp, _dp, _dp, _dp]
+    L.mhd_unit_ct_edge.argtypes = [ctypes.c_int, _dp, _dp]
     L.mhd_launch_count.restype = ctypes.c_longlong
     L.mhd_last_error.restype = ctypes.c_char_p
     for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_stream", "mhd_set_state",
                  "mhd_set_state_device", "mhd_compute_dt", "mhd_step", "mhd_advance", "mhd_get_state",
                  "mhd_get_state_device", "mhd_get_half_state", "mhd_max_divb", "mhd_synchronize",
-                 "mhd_finalize"):
+                 "mhd_finalize", "mhd_get_flux", "mhd_unit_hlld", "mhd_unit_reconstruct", "mhd_unit_ct_edge"):
         getattr(L, name).restype = ctypes.c_int
     return L
 
@@ -83,6 +88,39 @@ def measure_peaks(seconds=0.0):
     tf, bw = ctypes.c_double(), ctypes.c_double()
     _check(_lib.mhd_measure_peaks(ctypes.byref(tf), ctypes.byref(bw), float(seconds)))
     return tf.value, bw.value
+
+
+def unit_hlld(gamma, WL, WR, bx):
+    """n HLLD solves on the device: WL, WR (n,7), bx (n,) -> F (n,7)."""
+    WL = np.ascontiguousarray(WL, dtype=np.float64).reshape(-1, 7)
+    WR = np.ascontiguousarray(WR, dtype=np.float64).reshape(-1, 7)
+    bx = np.ascontiguousarray(bx, dtype=np.float64).reshape(-1)
+    n = WL.shape[0]
+    if WR.shape[0] != n or bx.shape[0] != n:
+        raise MhdError("unit_hlld: inconsistent lengths")
+    F = np.empty((n, 7))
+    _check(_lib.mhd_unit_hlld(n, float(gamma), _hp(WL), _hp(WR), _hp(bx), _hp(F)))
+    return F
+
+
+def unit_reconstruct(gamma, recon, Ws, bn0):
+    """n reconstructions on the device: Ws (n, 2*recon+1, 7), bn0 (n,) -> (Wlo, Whi), (n,7) each."""
+    Ws = np.ascontiguousarray(Ws, dtype=np.float64).reshape(-1, 2 * recon + 1, 7)
+    bn0 = np.ascontiguousarray(bn0, dtype=np.float64).reshape(-1)
+    n = Ws.shape[0]
+    if bn0.shape[0] != n:
+        raise MhdError("unit_reconstruct: inconsistent lengths")
+    lo, hi = np.empty((n, 7)), np.empty((n, 7))
+    _check(_lib.mhd_unit_reconstruct(n, float(gamma), int(recon), _hp(Ws), _hp(bn0), _hp(lo), _hp(hi)))
+    return lo, hi
+
+
+def unit_ct_edge(in12):
+    """n CT edge fields on the device: in12 (n,12) in the argument order of mhd_unit_ct_edge."""
+    in12 = np.ascontiguousarray(in12, dtype=np.float64).reshape(-1, 12)
+    out = np.empty(in12.shape[0])
+    _check(_lib.mhd_unit_ct_edge(in12.shape[0], _hp(in12), _hp(out)))
+    return out
 
 
 class Mhd:
@@ -180,6 +218,12 @@ class Mhd:
         n = ctypes.c_int()
         _check(_lib.mhd_step_profile(float(dt), max_entries, ms, names, ctypes.byref(n)))
         return [(names[i].decode(), ms[i]) for i in range(n.value)]
+
+    def get_flux(self, axis, comp):
+        """Corrector flux component on the lower `axis`-faces of the active cells, shape (nz, ny, nx)."""
+        out = np.empty((self.n[2], self.n[1], self.n[0]))
+        _check(_lib.mhd_get_flux(int(axis), int(comp), _hp(out)))
+        return out
 
     def max_divb(self):
         v = ctypes.c_double()

@@ -192,18 +192,34 @@ def test_riemann_other_axes_outflow(mhd, axis):
 
 
 def test_c4_blast_small(mhd):
-    """Shape of BASELINE.json configs[3] at 32^3: PPMC, strong shock, 20 steps; positivity and parity."""
+    """Shape of BASELINE.json configs[3] at 32^3: PPMC, strong shock, 20 steps.  Every step is a
+    one-step parity case from the oracle's own state (the limiters are discontinuous switches, so a
+    free-running pair may legitimately part ways at a tie; BASELINE.json asks 1e-12 per step and
+    1e-9 only for the smooth-wave run).  The free-running GPU state is checked for what is unique:
+    positivity, div B, point symmetry about the centre, and closeness to the oracle run."""
     p = inputs.blast(32, recon=2, n_steps=20)
     o, g = make_pair(mhd, p)
+    state = p.state
+    worst = 0.0
     for s in range(p.n_steps):
+        g.set_state(state)
         dt = o.compute_dt(p.cfl)
+        assert abs(g.compute_dt(p.cfl) - dt) <= 1e-13 * dt
         o.step(dt); g.step(dt)
-        if s == 0:
-            assert_close(g.get_state(), o.get_state(), TOL_STEP, "blast step 1")
-    out, ref = g.get_state(), o.get_state()
-    assert_close(out, ref, TOL_RUN, "blast 20 steps")
+        state = o.get_state()
+        worst = max(worst, assert_close(g.get_state(), state, TOL_STEP, "blast step %d" % (s + 1)))
+    ref = state
+    # free-running GPU
+    g.set_state(p.state)
+    for s in range(p.n_steps):
+        g.step(g.compute_dt(p.cfl))
+    out = g.get_state()
     assert np.min(out["rho"]) > 0.0 and np.all(np.isfinite(out["E"]))
     assert divb_normalised(out, p.n) <= TOL_DIVB
+    for f in ("rho", "E"):   # point symmetry about the box centre (T13)
+        assert np.max(np.abs(out[f] - out[f][::-1, ::-1, ::-1])) <= 1e-11 * np.max(np.abs(out[f]))
+    rd = rel_diff(out, ref)
+    assert max(rd.values()) <= 1e-9, "blast 20 steps free-running: %s" % rd
     o.close(); g.close()
 
 
