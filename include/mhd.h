@@ -156,6 +156,11 @@ int mhd_unit_reconstruct(int n, double gamma, int recon, const double *Ws, const
  * faces, and the reference field of the four cells around the edge. */
 int mhd_unit_ct_edge(int n, const double *in12, double *out);
 
+/* The kernels' own fp64 reciprocal (op 0), reciprocal square root (op 1) and square root (op 2)
+ * (csrc/mhd_math.cuh: hardware seed + two Newton steps, no slow path) on n HOST values x > 0
+ * (op 2 also accepts 0); tests bound their error in ulps against IEEE. */
+int mhd_unit_math(int n, int op, const double *x, double *y);
+
 /* Number of kernel launches issued by this library since mhd_init (for bench.py). */
 long long mhd_launch_count(void);
 

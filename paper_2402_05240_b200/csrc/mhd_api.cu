@@ -21,7 +21,8 @@ struct Context {
   Geo g;
   State8 U, Uh;
   Flux21 F;
-  Edge3 E;
+  Edge3 E;   // CT edge fields
+  Edge3 Er;  // cell-centred reference field, Eq. 18
   Scalars *sc = nullptr;
   cudaStream_t stream = 0;
   long long launches = 0;
@@ -75,11 +76,12 @@ bool make_geo(Geo &g, int nx, int ny, int nz, double gamma, int recon) {
   g.ntot = g.s[2] * g.N[2];
   for (int a = 0; a < 3; a++) { g.d[a] = 1.0 / g.n[a]; g.bc[a] = MHD_BC_PERIODIC; }
   g.gamma = gamma;
+  g.gm1inv = 1.0 / (gamma - 1.0);
   g.recon = recon;
   return true;
 }
 
-const int kNumArrays = 2 * NFIELD + 21 + 3;  // U, Uh, fluxes, edge fields
+const int kNumArrays = 2 * NFIELD + 21 + 3 + 3;  // U, half state, fluxes, edge fields, reference field
 
 size_t array_bytes(const Geo &g) { return ((size_t)g.ntot * sizeof(double) + 255) / 256 * 256; }
 
@@ -158,7 +160,7 @@ int step_kernels() {
   {
     long long plane = (long long)(pb.hi[0] - pb.lo[0] + 1) * (pb.hi[1] - pb.lo[1] + 1);
     dim3 grid(grid1(plane, 128).x, pb.hi[2] - pb.lo[2] + 1);
-    k_predictor_flux<<<grid, 128, 0, C.stream>>>(C.U, C.F, g, pb);
+    k_predictor_flux<<<grid, 128, 0, C.stream>>>(C.U, C.F, C.Er, g, pb);
     LAUNCH_CHECK("k_predictor_flux");
   }
   // Step 4: CT on indices [-1-r, n+r+1];  Step 5: half update of cells [-1-r, n+r]
@@ -168,11 +170,11 @@ int step_kernels() {
     Box eb = hb;
     for (int a = 0; a < 3; a++) eb.hi[a] += 1;
     long long plane = (long long)(eb.hi[0] - eb.lo[0] + 1) * (eb.hi[1] - eb.lo[1] + 1);
-    dim3 grid(grid1(plane, 128).x, eb.hi[2] - eb.lo[2] + 1);
-    k_ct<<<grid, 128, 0, C.stream>>>(C.U, C.F, C.E, g, eb);
+    dim3 grid(grid1(plane, 256).x, eb.hi[2] - eb.lo[2] + 1);
+    k_ct<<<grid, 256, 0, C.stream>>>(C.F, C.Er, C.E, g, eb);
     LAUNCH_CHECK("k_ct(predictor)");
     dim3 gridu(grid1(plane, 256).x, eb.hi[2] - eb.lo[2] + 1);
-    k_update<<<gridu, 256, 0, C.stream>>>(C.U, C.Uh, C.F, C.E, g, hb, C.sc, 0.5);
+    k_update<true><<<gridu, 256, 0, C.stream>>>(C.U, C.Uh, C.F, C.E, C.Er, g, hb, C.sc, 0.5);
     LAUNCH_CHECK("k_update(half)");
   }
   // Steps 6-7: reconstruction + HLLD from U^{n+1/2}
@@ -186,11 +188,11 @@ int step_kernels() {
     Box ab, eb;
     for (int a = 0; a < 3; a++) { ab.lo[a] = 0; ab.hi[a] = g.n[a] - 1; eb.lo[a] = 0; eb.hi[a] = g.n[a]; }
     long long plane = (long long)(g.n[0] + 1) * (g.n[1] + 1);
-    dim3 grid(grid1(plane, 128).x, g.n[2] + 1);
-    k_ct<<<grid, 128, 0, C.stream>>>(C.Uh, C.F, C.E, g, eb);
+    dim3 grid(grid1(plane, 256).x, g.n[2] + 1);
+    k_ct<<<grid, 256, 0, C.stream>>>(C.F, C.Er, C.E, g, eb);
     LAUNCH_CHECK("k_ct(corrector)");
     dim3 gridu(grid1(plane, 256).x, g.n[2] + 1);
-    k_update<<<gridu, 256, 0, C.stream>>>(C.U, C.U, C.F, C.E, g, ab, C.sc, 1.0);
+    k_update<false><<<gridu, 256, 0, C.stream>>>(C.U, C.U, C.F, C.E, C.Er, g, ab, C.sc, 1.0);
     LAUNCH_CHECK("k_update(full)");
   }
   return MHD_OK;
@@ -228,12 +230,13 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
   for (int a = 0; a < 3; a++)
     for (int c = 0; c < 7; c++) { C.F.f[a][c] = (double *)p; p += ab; }
   for (int a = 0; a < 3; a++) { C.E.f[a] = (double *)p; p += ab; }
+  for (int a = 0; a < 3; a++) { C.Er.f[a] = (double *)p; p += ab; }
   C.launches = 0;
   C.inited = true;
   cudaError_t e = cudaMemsetAsync(C.base, 0, need, C.stream);
   if (e != cudaSuccess) { mhd_finalize(); return cuda_fail(e, "cudaMemsetAsync"); }
-  k_reset_min<<<1, 1, 0, C.stream>>>(C.sc);
-  LAUNCH_CHECK("k_reset_min");
+  k_reset_rate<<<1, 1, 0, C.stream>>>(C.sc);
+  LAUNCH_CHECK("k_reset_rate");
   return MHD_OK;
 }
 
@@ -329,12 +332,12 @@ int mhd_compute_dt(double cfl, double *dt) {
   if (rc) return rc;
   Scalars h;
   CU(cudaMemcpyAsync(&h, C.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, C.stream));
-  k_reset_min<<<1, 1, 0, C.stream>>>(C.sc);
-  LAUNCH_CHECK("k_reset_min");
+  k_reset_rate<<<1, 1, 0, C.stream>>>(C.sc);
+  LAUNCH_CHECK("k_reset_rate");
   CU(cudaStreamSynchronize(C.stream));
   double m;
-  memcpy(&m, &h.min_bits, sizeof(double));
-  *dt = cfl * m;
+  memcpy(&m, &h.rate_bits, sizeof(double));
+  *dt = cfl / m;
   if (h.bad) return fail(MHD_ERR_UNPHYSICAL, "non-physical state (rho <= 0, P <= 0 or non-finite)");
   return MHD_OK;
 }
@@ -395,7 +398,16 @@ int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *
                        double *by, double *bz) {
   if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
   double *dst[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
-  int rc = get_state_to(C.Uh, dst, true);
+  // the half state is held as (rho, v, P, face B): convert to the ABI's conserved variables in
+  // scratch (x-flux arrays 0..4 are free after the step; get_state_to stages through others)
+  const Geo &g = C.g;
+  State8 tmp = C.Uh;
+  for (int f = 0; f < 5; f++) tmp.f[f] = C.F.f[2][f];
+  Box ab = make_box(0, g.n[0] - 1, 0, g.n[1] - 1, 0, g.n[2] - 1);
+  long long plane = (long long)g.n[0] * g.n[1];
+  k_half_to_cons<<<dim3(grid1(plane, 256).x, g.n[2]), 256, 0, C.stream>>>(C.Uh, tmp, g, ab);
+  LAUNCH_CHECK("k_half_to_cons");
+  int rc = get_state_to(tmp, dst, true);
   if (rc) return rc;
   CU(cudaStreamSynchronize(C.stream));
   return MHD_OK;
@@ -442,7 +454,7 @@ int mhd_step_profile(double dt, int max_entries, double *ms, const char **names,
   cudaEventRecord(C.prof_ev[0], C.stream);
   int rc = cfl_kernel();
   if (!rc) {
-    k_reset_min<<<1, 1, 0, C.stream>>>(C.sc);
+    k_reset_rate<<<1, 1, 0, C.stream>>>(C.sc);
     C.launches++;
     rc = step_kernels();
   }

@@ -10,6 +10,8 @@
 #include <cuda_runtime.h>
 #include <math.h>
 
+#include "mhd_math.cuh"
+
 namespace mhd {
 
 struct W7 {
@@ -20,54 +22,64 @@ struct F7 {  // mass, mom_n, mom_t1, mom_t2, energy, By-flux, Bz-flux
   double m, mn, mt1, mt2, e, by, bz;
 };
 
-// Eq. 12: c_f^2 along the direction whose field component is bn.
+// Eq. 12: c_f^2 along the direction whose field component is bn; irho = 1/rho.
 // The discriminant is clamped at 0 against round-off (reading R3).
-__device__ __forceinline__ double fast_speed_sq(double gamma, double rho, double P, double bn,
+__device__ __forceinline__ double fast_speed_sq(double gamma, double irho, double P, double bn,
                                                 double bt1, double bt2) {
   double gp = gamma * P;
   double b2 = bn * bn + bt1 * bt1 + bt2 * bt2;
   double s = gp + b2;
   double disc = s * s - 4.0 * gp * bn * bn;
   disc = disc < 0.0 ? 0.0 : disc;
-  return (s + sqrt(disc)) / (2.0 * rho);
+  return (s + sqrt_(disc)) * (0.5 * irho);
 }
 
 // ---------------------------------------------------------------------------------------
 // HLLD (Miyoshi & Kusano 2005, cited PAPER.md:149; reading O4, wave speeds G15).
+// Work is kept to what the selected branch needs: total pressure / energy of both sides and both
+// single-star states always (S_M, p_T* and the double-star state need them), the physical flux
+// only of the side that bounds the face.  Seven reciprocals and three square roots per solve.
 // ---------------------------------------------------------------------------------------
 struct HlldSide {
-  double rho, u, v, w, by, bz;  // primitive inputs
-  double pT, e;                 // total pressure, total energy density
-  double Fm, Fmn, Fmt1, Fmt2, Fe, Fby, Fbz;  // physical flux, Eq. 8
-  double rhos, vs, ws, bys, bzs, es;         // single-star state
+  double rho, u, v, w, by, bz;        // primitive inputs
+  double pT, e;                       // total pressure, total energy density
+  double rhos, vs, ws, bys, bzs, es;  // single-star state
 };
 
-__device__ __forceinline__ void hlld_side_init(HlldSide &s, const W7 &W, double bx, double gm1inv,
-                                               double &P) {
-  s.rho = W.rho; s.u = W.u; s.v = W.v; s.w = W.w; s.by = W.by; s.bz = W.bz; P = W.P;
+__device__ __forceinline__ void hlld_side_init(HlldSide &s, const W7 &W, double bx, double gm1inv) {
+  s.rho = W.rho; s.u = W.u; s.v = W.v; s.w = W.w; s.by = W.by; s.bz = W.bz;
   double b2 = bx * bx + W.by * W.by + W.bz * W.bz;
   s.pT = W.P + 0.5 * b2;
   s.e = W.P * gm1inv + 0.5 * W.rho * (W.u * W.u + W.v * W.v + W.w * W.w) + 0.5 * b2;
-  s.Fm = W.rho * W.u;
-  s.Fmn = W.rho * W.u * W.u + s.pT - bx * bx;
-  s.Fmt1 = W.rho * W.u * W.v - bx * W.by;
-  s.Fmt2 = W.rho * W.u * W.w - bx * W.bz;
-  s.Fe = W.u * (s.e + s.pT) - bx * (W.u * bx + W.v * W.by + W.w * W.bz);
-  s.Fby = W.by * W.u - bx * W.v;
-  s.Fbz = W.bz * W.u - bx * W.w;
+}
+
+// Eq. 8 without the zero row
+__device__ __forceinline__ F7 phys_flux(const HlldSide &s, double bx) {
+  F7 F;
+  double ru = s.rho * s.u;
+  F.m = ru;
+  F.mn = ru * s.u + s.pT - bx * bx;
+  F.mt1 = ru * s.v - bx * s.by;
+  F.mt2 = ru * s.w - bx * s.bz;
+  F.e = s.u * (s.e + s.pT) - bx * (s.u * bx + s.v * s.by + s.w * s.bz);
+  F.by = s.by * s.u - bx * s.v;
+  F.bz = s.bz * s.u - bx * s.w;
+  return F;
 }
 
 // single-star state of one side (M&K Eq. 43-48); S = outer speed of this side
 __device__ __forceinline__ void hlld_star(HlldSide &s, double S, double SM, double pTs, double bx) {
   double Su = S - s.u;
   double SSm = S - SM;
-  double iSSm = 1.0 / SSm;
-  s.rhos = s.rho * (Su * iSSm);
   double D = s.rho * Su * SSm - bx * bx;
+  double iSSm;
   if (fabs(D) < 1e-8 * pTs) {  // degenerate 0/0: no jump in the tangential fields
+    iSSm = rcp(SSm);
     s.vs = s.v; s.ws = s.w; s.bys = s.by; s.bzs = s.bz;
   } else {
-    double iD = 1.0 / D;
+    double inv = rcp(D * SSm);  // one reciprocal for 1/D and 1/(S - S_M)
+    double iD = inv * SSm;
+    iSSm = inv * D;
     double fv = bx * (SM - s.u) * iD;
     double fb = (s.rho * Su * Su - bx * bx) * iD;
     s.vs = s.v - s.by * fv;
@@ -75,74 +87,75 @@ __device__ __forceinline__ void hlld_star(HlldSide &s, double S, double SM, doub
     s.bys = s.by * fb;
     s.bzs = s.bz * fb;
   }
+  s.rhos = s.rho * (Su * iSSm);
   double vb = s.u * bx + s.v * s.by + s.w * s.bz;
   double vbs = SM * bx + s.vs * s.bys + s.ws * s.bzs;
   s.es = (Su * s.e - s.pT * s.u + pTs * SM + bx * (vb - vbs)) * iSSm;
 }
 
-__device__ __forceinline__ F7 hlld(double gamma, const W7 &WL, const W7 &WR, double bx) {
+// irL, irR = 1/rho of the two states (the callers have them or form them once)
+__device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, const W7 &WR, double irL,
+                                   double irR, double bx) {
   HlldSide L, R;
-  double PL, PR;
-  double gm1inv = 1.0 / (gamma - 1.0);
-  hlld_side_init(L, WL, bx, gm1inv, PL);
-  hlld_side_init(R, WR, bx, gm1inv, PR);
-  double cfL = sqrt(fast_speed_sq(gamma, L.rho, PL, bx, L.by, L.bz));
-  double cfR = sqrt(fast_speed_sq(gamma, R.rho, PR, bx, R.by, R.bz));
-  double cfmax = fmax(cfL, cfR);
+  hlld_side_init(L, WL, bx, gm1inv);
+  hlld_side_init(R, WR, bx, gm1inv);
+  double cf2L = fast_speed_sq(gamma, irL, WL.P, bx, L.by, L.bz);
+  double cf2R = fast_speed_sq(gamma, irR, WR.P, bx, R.by, R.bz);
+  double cfmax = sqrt_(fmax(cf2L, cf2R));
   double SL = fmin(L.u, R.u) - cfmax;
   double SR = fmax(L.u, R.u) + cfmax;
 
-  F7 F;
-  if (SL > 0.0) {
-    F.m = L.Fm; F.mn = L.Fmn; F.mt1 = L.Fmt1; F.mt2 = L.Fmt2; F.e = L.Fe; F.by = L.Fby; F.bz = L.Fbz;
-    return F;
-  }
-  if (SR < 0.0) {
-    F.m = R.Fm; F.mn = R.Fmn; F.mt1 = R.Fmt1; F.mt2 = R.Fmt2; F.e = R.Fe; F.by = R.Fby; F.bz = R.Fbz;
-    return F;
-  }
+  if (SL > 0.0) return phys_flux(L, bx);
+  if (SR < 0.0) return phys_flux(R, bx);
+
   // middle wave and total pressure of the fan (M&K Eq. 38, 41)
   double sduL = (SL - L.u) * L.rho;
   double sduR = (SR - R.u) * R.rho;
-  double iden = 1.0 / (sduR - sduL);
+  double iden = rcp(sduR - sduL);
   double SM = (sduR * R.u - sduL * L.u - R.pT + L.pT) * iden;
   double pTs = (sduR * L.pT - sduL * R.pT + L.rho * R.rho * (SR - R.u) * (SL - L.u) * (R.u - L.u)) * iden;
 
   hlld_star(L, SL, SM, pTs, bx);
   hlld_star(R, SR, SM, pTs, bx);
-  double rL = sqrt(L.rhos), rR = sqrt(R.rhos);
+  double rL, rR, irsL, irsR;
+  sqrt_rsqrt(L.rhos, rL, irsL);
+  sqrt_rsqrt(R.rhos, rR, irsR);
   double abx = fabs(bx);
-  double SsL = SM - abx / rL;
-  double SsR = SM + abx / rR;
+  double SsL = SM - abx * irsL;
+  double SsR = SM + abx * irsR;
 
   // side whose states bound the face: left if S_M >= 0 (S*_L >= 0 implies S_M >= 0)
-  bool left = (SM >= 0.0);
-  bool dbl = left ? !(SsL >= 0.0) : !(SsR <= 0.0);
-  const HlldSide &a = left ? L : R;
-  double S = left ? SL : SR;
-  double Ss = left ? SsL : SsR;
-  double Um = a.rho, Umn = a.rho * a.u, Umt1 = a.rho * a.v, Umt2 = a.rho * a.w;
-  double Usm = a.rhos, Usmn = a.rhos * SM, Usmt1 = a.rhos * a.vs, Usmt2 = a.rhos * a.ws;
+  const bool left = (SM >= 0.0);
+  const bool dbl = left ? !(SsL >= 0.0) : !(SsR <= 0.0);
+  HlldSide a;
+  a.rho = left ? L.rho : R.rho; a.u = left ? L.u : R.u; a.v = left ? L.v : R.v; a.w = left ? L.w : R.w;
+  a.by = left ? L.by : R.by; a.bz = left ? L.bz : R.bz; a.pT = left ? L.pT : R.pT; a.e = left ? L.e : R.e;
+  a.rhos = left ? L.rhos : R.rhos; a.vs = left ? L.vs : R.vs; a.ws = left ? L.ws : R.ws;
+  a.bys = left ? L.bys : R.bys; a.bzs = left ? L.bzs : R.bzs; a.es = left ? L.es : R.es;
+  const double S = left ? SL : SR;
+  F7 F = phys_flux(a, bx);
+  const double Usmt1 = a.rhos * a.vs, Usmt2 = a.rhos * a.ws;
   // F*_a = F_a + S_a (U*_a - U_a)
-  F.m = a.Fm + S * (Usm - Um);
-  F.mn = a.Fmn + S * (Usmn - Umn);
-  F.mt1 = a.Fmt1 + S * (Usmt1 - Umt1);
-  F.mt2 = a.Fmt2 + S * (Usmt2 - Umt2);
-  F.e = a.Fe + S * (a.es - a.e);
-  F.by = a.Fby + S * (a.bys - a.by);
-  F.bz = a.Fbz + S * (a.bzs - a.bz);
+  F.m += S * (a.rhos - a.rho);
+  F.mn += S * (a.rhos * SM - a.rho * a.u);
+  F.mt1 += S * (Usmt1 - a.rho * a.v);
+  F.mt2 += S * (Usmt2 - a.rho * a.w);
+  F.e += S * (a.es - a.e);
+  F.by += S * (a.bys - a.by);
+  F.bz += S * (a.bzs - a.bz);
   if (dbl) {
     // double-star states (M&K Eq. 59-63)
+    const double Ss = left ? SsL : SsR;
     double sgn = (bx > 0.0) ? 1.0 : ((bx < 0.0) ? -1.0 : 0.0);
-    double inv = 1.0 / (rL + rR);
+    double inv = rcp(rL + rR);
     double vss = (rL * L.vs + rR * R.vs + (R.bys - L.bys) * sgn) * inv;
     double wss = (rL * L.ws + rR * R.ws + (R.bzs - L.bzs) * sgn) * inv;
     double byss = (rL * R.bys + rR * L.bys + rL * rR * (R.vs - L.vs) * sgn) * inv;
     double bzss = (rL * R.bzs + rR * L.bzs + rL * rR * (R.ws - L.ws) * sgn) * inv;
     double vbss = SM * bx + vss * byss + wss * bzss;
     double vbs = SM * bx + a.vs * a.bys + a.ws * a.bzs;
-    double r = left ? rL : rR;
-    double ess = left ? a.es - r * (vbs - vbss) * sgn : a.es + r * (vbs - vbss) * sgn;
+    double r = left ? -rL : rR;
+    double ess = a.es + r * (vbs - vbss) * sgn;
     // F**_a = F*_a + S*_a (U**_a - U*_a); rho** = rho*, u** = S_M
     F.mt1 += Ss * (a.rhos * vss - Usmt1);
     F.mt2 += Ss * (a.rhos * wss - Usmt2);
@@ -179,33 +192,40 @@ struct C7 {  // characteristic amplitudes
 
 __device__ __forceinline__ void eig_setup(Eig &e, double gamma, const W7 &W, double bx) {
   double rho = W.rho;
-  double irho = 1.0 / rho;
-  double a2 = gamma * W.P * irho;
-  double a = sqrt(a2);
-  double cf2 = fast_speed_sq(gamma, rho, W.P, bx, W.by, W.bz);
+  double sr, isr;
+  sqrt_rsqrt(rho, sr, isr);
+  double irho = isr * isr;
+  double gp = gamma * W.P;
+  double a2 = gp * irho;
+  double a, ia;
+  sqrt_rsqrt(a2, a, ia);
+  double ia2 = ia * ia;
+  double bp2 = W.by * W.by + W.bz * W.bz;
+  double s = gp + (bx * bx + bp2);
+  double disc = s * s - 4.0 * gp * bx * bx;
+  disc = disc < 0.0 ? 0.0 : disc;                 // reading R3
+  double cf2 = (s + sqrt_(disc)) * (0.5 * irho);  // Eq. 12
   double ca2 = bx * bx * irho;
-  double cs2 = (cf2 > 0.0) ? a2 * ca2 / cf2 : 0.0;
-  double cf = sqrt(cf2), cs = sqrt(cs2);
-  double bperp = sqrt(W.by * W.by + W.bz * W.bz);
-  if (bperp == 0.0) { e.betay = 1.0; e.betaz = 0.0; }
-  else { double ib = 1.0 / bperp; e.betay = W.by * ib; e.betaz = W.bz * ib; }
+  double cs2 = (cf2 > 0.0) ? a2 * ca2 * rcp(cf2) : 0.0;  // slow speed without cancellation (O9)
+  double cf = sqrt_(cf2), cs = sqrt_(cs2);
+  if (bp2 == 0.0) { e.betay = 1.0; e.betaz = 0.0; }
+  else { double ib = rsqrt_(bp2); e.betay = W.by * ib; e.betaz = W.bz * ib; }
   double dfs = cf2 - cs2;
   if (dfs == 0.0) { e.alf = 1.0; e.als = 0.0; }
   else {
-    double idfs = 1.0 / dfs;
+    double idfs = rcp(dfs);
     double af2 = (a2 - cs2) * idfs;
     double as2 = (cf2 - a2) * idfs;
     af2 = af2 < 0.0 ? 0.0 : (af2 > 1.0 ? 1.0 : af2);
     as2 = as2 < 0.0 ? 0.0 : (as2 > 1.0 ? 1.0 : as2);
-    e.alf = sqrt(af2); e.als = sqrt(as2);
+    e.alf = sqrt_(af2); e.als = sqrt_(as2);
   }
   double S = (bx >= 0.0) ? 1.0 : -1.0;
-  double sr = sqrt(rho);
-  e.rho = rho; e.irho = irho; e.a2 = a2; e.ia2 = 1.0 / a2; e.N = 0.5 * e.ia2;
+  e.rho = rho; e.irho = irho; e.a2 = a2; e.ia2 = ia2; e.N = 0.5 * ia2;
   e.Cff = cf * e.alf; e.Css = cs * e.als;
   e.Qf = e.Cff * S; e.Qs = e.Css * S;
   e.Af = a * e.alf * sr; e.As = a * e.als * sr;
-  e.Ssr = S * sr; e.Sisr = S / sr;
+  e.Ssr = S * sr; e.Sisr = S * isr;
 }
 
 // a = L . x   (x in the component order of W7).  Written with explicit rounding intrinsics so

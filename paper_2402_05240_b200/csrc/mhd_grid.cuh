@@ -34,6 +34,7 @@ struct Geo {
   long long ntot;  // pitch * N[1] * N[2]
   double d[3];     // Delta_a = 1/n_a
   double gamma;
+  double gm1inv;   // 1 / (gamma - 1)
   int bc[3];
   int recon;
 };
@@ -47,29 +48,49 @@ __device__ __forceinline__ long long cell_index(const Geo &g, int i, int j, int 
 }
 
 struct Prim {
-  double rho, v[3], P, B[3];
+  double rho, ir, v[3], P, B[3];  // ir = 1/rho
 };
 
-// O1: v = m / rho, cell-centred B = mean of the two opposing faces
-// (Eq. 13), P from the total energy.  Primitives are recomputed wherever needed, never stored
-// (PAPER.md:305).
+// P = (gamma-1)(E - rho v^2/2 - B^2/2) with explicit roundings: every inlined copy
+// is the same instruction sequence, so bit-identical cells give bit-identical pressures (the
+// limiters' "<= 0" tests include equality, O10; reading R8).
+__device__ __forceinline__ double pressure(double gm1, double rho, const double v[3], double E,
+                                           const double B[3]) {
+  double v2 = __fma_rn(v[2], v[2], __fma_rn(v[1], v[1], __dmul_rn(v[0], v[0])));
+  double b2 = __fma_rn(B[2], B[2], __fma_rn(B[1], B[1], __dmul_rn(B[0], B[0])));
+  double ek = __dmul_rn(__dmul_rn(0.5, rho), v2);
+  return __dmul_rn(gm1, __fma_rn(-0.5, b2, __dadd_rn(E, -ek)));
+}
+
+// O1 from the CONSERVED state U^n: v = m / rho, cell-centred B = mean of
+// the two opposing faces (Eq. 13), P from the total energy.
 __device__ __forceinline__ Prim load_prim(const State8 &U, const Geo &g, long long idx) {
   Prim p;
   double rho = __ldg(U.f[F_RHO] + idx);
-  double ir = 1.0 / rho;
-  p.rho = rho;
+  double ir = rcp(rho);
+  p.rho = rho; p.ir = ir;
 #pragma unroll
   for (int a = 0; a < 3; a++) {
     p.B[a] = 0.5 * (__ldg(U.f[F_BX + a] + idx) + __ldg(U.f[F_BX + a] + idx + g.s[a]));
     p.v[a] = __ldg(U.f[F_MX + a] + idx) * ir;
   }
-  double E = __ldg(U.f[F_E] + idx);
-  // explicit roundings: every inlined copy is the same instruction sequence, so bit-identical
-  // cells give bit-identical primitives (the limiters' "<= 0" tests include equality, O10)
-  double v2 = __fma_rn(p.v[2], p.v[2], __fma_rn(p.v[1], p.v[1], __dmul_rn(p.v[0], p.v[0])));
-  double b2 = __fma_rn(p.B[2], p.B[2], __fma_rn(p.B[1], p.B[1], __dmul_rn(p.B[0], p.B[0])));
-  double ek = __dmul_rn(__dmul_rn(0.5, rho), v2);
-  p.P = __dmul_rn(g.gamma - 1.0, __fma_rn(-0.5, b2, __dadd_rn(E, -ek)));
+  p.P = pressure(g.gamma - 1.0, rho, p.v, __ldg(U.f[F_E] + idx), p.B);
+  return p;
+}
+
+// The half-step state is held in PRIMITIVE form (rho, v, P at cell centres in slots F_RHO..F_E,
+// face B^{n+1/2} in slots F_BX..F_BZ): the three sweep kernels and the CT kernel of the corrector
+// read it ready-made instead of each redoing the division and the pressure.
+__device__ __forceinline__ Prim load_prim_half(const State8 &Wh, const Geo &g, long long idx) {
+  Prim p;
+  p.rho = __ldg(Wh.f[F_RHO] + idx);
+  p.ir = 0.0;  // not stored; formed where needed
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    p.B[a] = 0.5 * (__ldg(Wh.f[F_BX + a] + idx) + __ldg(Wh.f[F_BX + a] + idx + g.s[a]));
+    p.v[a] = __ldg(Wh.f[F_MX + a] + idx);
+  }
+  p.P = __ldg(Wh.f[F_E] + idx);
   return p;
 }
 

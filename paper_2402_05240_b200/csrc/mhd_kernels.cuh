@@ -83,82 +83,99 @@ __global__ void k_pack(double *__restrict__ dst, const double *__restrict__ src,
 }
 
 // ---------------------------------------------------------------------------------------
-// a1: CFL.  Positive doubles order like their bit patterns, so the grid-wide minimum is an
-// unsigned 64-bit atomicMin (the integer-encoding idea of PAPER.md:325, without the sign
-// handling the paper's max needs).  Scalars: sc[0] = bits of the running minimum,
-// sc[1] = dt, sc[2] = accumulated time, sc[3] = bad-state flag (as double bits != 0).
+// a1: CFL.  Each thread forms the largest signal rate (|v_a| + c_f,a) / Delta_a of its cell; the
+// grid-wide maximum goes through warp shuffles, shared memory and one atomic per block
+// (PAPER.md:317-327).  Positive doubles order like their bit patterns, so the atomic is an
+// unsigned 64-bit atomicMax (the integer-encoding idea of PAPER.md:325 without the sign
+// handling).  dt = cfl / max rate  (= cfl * min Delta_a / (|v_a| + c_f,a), Eq. 11).
 // ---------------------------------------------------------------------------------------
 struct Scalars {
-  unsigned long long min_bits;
+  unsigned long long rate_bits;  // running maximum of the signal rate
   double dt;
   double t_accum;
   unsigned long long bad;
 };
 
-__device__ __forceinline__ double warp_min(double v) {
+__device__ __forceinline__ double warp_max(double v) {
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
   return v;
 }
 
-__global__ void __launch_bounds__(256) k_cfl(State8 U, Geo g, Scalars *sc) {
-  __shared__ double wmin[8];
-  __shared__ int wbad[8];
-  const int plane = g.n[0] * g.n[1];
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
-  const int k = blockIdx.y;
-  double tmin = INFINITY;
-  int bad = 0;
-  if (t < plane) {
-    int i = t % g.n[0], j = t / g.n[0];
-    Prim p = load_prim(U, g, cell_index(g, i, j, k));
-    bad = !(p.rho > 0.0) || !(p.P > 0.0) || !isfinite(p.rho) || !isfinite(p.P);
+__device__ __forceinline__ double cell_rate(const Geo &g, const Prim &p, int &bad) {
+  bad |= !(p.rho > 0.0) || !(p.P > 0.0) || !isfinite(p.rho) || !isfinite(p.P);
+  double r = 0.0;
 #pragma unroll
-    for (int a = 0; a < 3; a++) {
-      double cf = sqrt(fast_speed_sq(g.gamma, p.rho, p.P, p.B[a], p.B[(a + 1) % 3], p.B[(a + 2) % 3]));
-      double tt = g.d[a] / (fabs(p.v[a]) + cf);
-      if (!isfinite(tt)) bad = 1;
-      tmin = fmin(tmin, tt);
-    }
+  for (int a = 0; a < 3; a++) {
+    double cf = sqrt_(fast_speed_sq(g.gamma, p.ir, p.P, p.B[a], p.B[(a + 1) % 3], p.B[(a + 2) % 3]));
+    r = fmax(r, (fabs(p.v[a]) + cf) * (double)g.n[a]);  // 1/Delta_a = n_a exactly (unit box)
   }
-  tmin = warp_min(tmin);
+  bad |= !isfinite(r) || !(r > 0.0);
+  return r;
+}
+
+__device__ __forceinline__ void block_rate_reduce(double r, int bad, Scalars *sc) {
+  __shared__ double wmax[32];
+  __shared__ int wbad[32];
+  r = warp_max(r);
   bad = __any_sync(0xffffffffu, bad);
-  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  if (l == 0) { wmin[w] = tmin; wbad[w] = bad; }
+  const int t = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+  const int nt = blockDim.x * blockDim.y * blockDim.z;
+  const int w = t >> 5, l = t & 31;
+  if (l == 0) { wmax[w] = r; wbad[w] = bad; }
   __syncthreads();
   if (w == 0) {
-    int nw = blockDim.x >> 5;
-    tmin = (l < nw) ? wmin[l] : INFINITY;
+    int nw = (nt + 31) >> 5;
+    r = (l < nw) ? wmax[l] : 0.0;
     bad = (l < nw) ? wbad[l] : 0;
-    tmin = warp_min(tmin);
+    r = warp_max(r);
     bad = __any_sync(0xffffffffu, bad);
     if (l == 0) {
-      if (tmin > 0.0 && tmin < INFINITY)
-        atomicMin(&sc->min_bits, (unsigned long long)__double_as_longlong(tmin));
+      if (r > 0.0 && r < INFINITY) atomicMax(&sc->rate_bits, (unsigned long long)__double_as_longlong(r));
       if (bad) atomicOr(&sc->bad, 1ull);
     }
   }
 }
 
-__global__ void k_reset_min(Scalars *sc) {
-  sc->min_bits = (unsigned long long)__double_as_longlong(INFINITY);
+__global__ void __launch_bounds__(256) k_cfl(State8 U, Geo g, Scalars *sc) {
+  const int plane = g.n[0] * g.n[1];
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int k = blockIdx.y;
+  double r = 0.0;
+  int bad = 0;
+  if (t < plane) {
+    int i = t % g.n[0], j = t / g.n[0];
+    Prim p = load_prim(U, g, cell_index(g, i, j, k));
+    r = cell_rate(g, p, bad);
+  }
+  block_rate_reduce(r, bad, sc);
 }
 
-// dt = cfl * min; accumulate time; re-arm the reduction
+__global__ void k_reset_rate(Scalars *sc) { sc->rate_bits = 0ull; }
+
+// dt = cfl / max rate; accumulate time; re-arm the reduction
 __global__ void k_finish_dt(Scalars *sc, double cfl) {
-  double m = __longlong_as_double((long long)sc->min_bits);
-  sc->dt = cfl * m;
+  double m = __longlong_as_double((long long)sc->rate_bits);
+  sc->dt = cfl / m;
   sc->t_accum += sc->dt;
-  sc->min_bits = (unsigned long long)__double_as_longlong(INFINITY);
+  sc->rate_bits = 0ull;
 }
 
 __global__ void k_set_dt(Scalars *sc, double dt) { sc->dt = dt; }
+
+// Eq. 18: cell-centred reference field E = -(v x B)
+__device__ __forceinline__ void store_eref(const Edge3 &Er, long long idx, const Prim &p) {
+  Er.f[0][idx] = -(p.v[1] * p.B[2] - p.v[2] * p.B[1]);
+  Er.f[1][idx] = -(p.v[2] * p.B[0] - p.v[0] * p.B[2]);
+  Er.f[2][idx] = -(p.v[0] * p.B[1] - p.v[1] * p.B[0]);
+}
 
 // ---------------------------------------------------------------------------------------
 // a2: predictor.  One thread per cell of `box`; it forms the PCM states (Eq. 14)
 // of its own cell and of its three lower neighbours and solves HLLD on its three lower faces
 // (fused PCM+HLLD, the paper's K1).  B_n is the face value.
-// Face a is skipped where the lower neighbour lies outside the box.
+// Face a is skipped where the lower neighbour lies outside the box.  The thread also leaves
+// the reference field of its cell (Eq. 18) for the CT kernel.
 // ---------------------------------------------------------------------------------------
 template <int A>
 __device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const Geo &g,
@@ -167,26 +184,27 @@ __device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const
   double bn;
   W7 WL = to_W<A>(pm, bn);
   W7 WR = to_W<A>(pc, bn);
-  F7 f = hlld(g.gamma, WL, WR, __ldg(U.f[F_BX + A] + idx));
+  F7 f = hlld(g.gamma, g.gm1inv, WL, WR, pm.ir, pc.ir, __ldg(U.f[F_BX + A] + idx));
   store_flux<A>(F, idx, f);
 }
 
 #ifndef MHD_MINB_PRED
-#define MHD_MINB_PRED 1
+#define MHD_MINB_PRED 4
 #endif
 #ifndef MHD_MINB_FX
-#define MHD_MINB_FX 1
+#define MHD_MINB_FX 4
 #endif
 #ifndef MHD_MINB_FM
-#define MHD_MINB_FM 1
+#define MHD_MINB_FM 4
 #endif
-__global__ void __launch_bounds__(128, MHD_MINB_PRED) k_predictor_flux(State8 U, Flux21 F, Geo g, Box box) {
+__global__ void __launch_bounds__(128, MHD_MINB_PRED) k_predictor_flux(State8 U, Flux21 F, Edge3 Er, Geo g, Box box) {
   const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= lx * ly) return;
   int i = box.lo[0] + t % lx, j = box.lo[1] + t / lx, k = box.lo[2] + blockIdx.y;
   long long idx = cell_index(g, i, j, k);
   Prim pc = load_prim(U, g, idx);
+  store_eref(Er, idx, pc);
   if (i > box.lo[0]) pcm_face<0>(U, F, g, idx, pc);
   if (j > box.lo[1]) pcm_face<1>(U, F, g, idx, pc);
   if (k > box.lo[2]) pcm_face<2>(U, F, g, idx, pc);
@@ -196,67 +214,55 @@ __global__ void __launch_bounds__(128, MHD_MINB_PRED) k_predictor_flux(State8 U,
 // a3 / a7: CT.  One thread per index of `box`; it evaluates the three edges on the lower
 // corner of its cell.  Face E from the magnetic fluxes per Table 1 (O5):
 // on an a-face E_c = -F_a[B_t1], on a b-face E_c = +F_b[B_t2], (a,b,c) cyclic.  The
-// cell-centred reference field is Eq. 18 from the state `U` handed in (U^n or U^{n+1/2}).
+// cell-centred reference field (Eq. 18) was left in `Er` by the kernel that produced the state
+// (predictor: U^n; half update: U^{n+1/2}), so this kernel is pure stencil traffic.
 // ---------------------------------------------------------------------------------------
-struct VB {
-  double v[3], B[3];
-};
-
-__device__ __forceinline__ VB load_vb(const State8 &U, const Geo &g, long long idx) {
-  VB q;
-  double ir = 1.0 / __ldg(U.f[F_RHO] + idx);
-#pragma unroll
-  for (int a = 0; a < 3; a++) {
-    q.v[a] = __ldg(U.f[F_MX + a] + idx) * ir;
-    q.B[a] = 0.5 * (__ldg(U.f[F_BX + a] + idx) + __ldg(U.f[F_BX + a] + idx + g.s[a]));
-  }
-  return q;
-}
-
 template <int C>
-__device__ __forceinline__ double eref(const VB &q) {  // Eq. 18: -(v x B)_c
-  constexpr int A = (C + 1) % 3, B = (C + 2) % 3;
-  return -(q.v[A] * q.B[B] - q.v[B] * q.B[A]);
-}
-
-template <int C>
-__device__ __forceinline__ void ct_one(const Flux21 &F, const Edge3 &E, const Geo &g, long long idx,
-                                       const VB &q00, const VB &q10, const VB &q01, const VB &q11) {
+__device__ __forceinline__ void ct_one(const Flux21 &F, const Edge3 &Er, const Edge3 &E, const Geo &g,
+                                       long long idx) {
   constexpr int A = (C + 1) % 3, B = (C + 2) % 3;
   const long long sa = g.s[A], sb = g.s[B];
   double Ea0 = -__ldg(F.f[A][5] + idx), Ea1 = -__ldg(F.f[A][5] + idx - sb);
   double Eb0 = __ldg(F.f[B][6] + idx), Eb1 = __ldg(F.f[B][6] + idx - sa);
   double Ma0 = __ldg(F.f[A][0] + idx), Ma1 = __ldg(F.f[A][0] + idx - sb);
   double Mb0 = __ldg(F.f[B][0] + idx), Mb1 = __ldg(F.f[B][0] + idx - sa);
-  E.f[C][idx] = ct_edge(Ea0, Ea1, Eb0, Eb1, Ma0, Ma1, Mb0, Mb1, eref<C>(q00), eref<C>(q10),
-                        eref<C>(q01), eref<C>(q11));
+  const double *er = Er.f[C];
+  E.f[C][idx] = ct_edge(Ea0, Ea1, Eb0, Eb1, Ma0, Ma1, Mb0, Mb1, __ldg(er + idx), __ldg(er + idx - sa),
+                        __ldg(er + idx - sb), __ldg(er + idx - sa - sb));
 }
 
-__global__ void __launch_bounds__(128) k_ct(State8 U, Flux21 F, Edge3 E, Geo g, Box box) {
+__global__ void __launch_bounds__(256) k_ct(Flux21 F, Edge3 Er, Edge3 E, Geo g, Box box) {
   const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= lx * ly) return;
   int i = box.lo[0] + t % lx, j = box.lo[1] + t / lx, k = box.lo[2] + blockIdx.y;
   long long idx = cell_index(g, i, j, k);
-  const long long sx = g.s[0], sy = g.s[1], sz = g.s[2];
-  VB c = load_vb(U, g, idx);
-  VB cx = load_vb(U, g, idx - sx), cy = load_vb(U, g, idx - sy), cz = load_vb(U, g, idx - sz);
-  VB cxy = load_vb(U, g, idx - sx - sy), cyz = load_vb(U, g, idx - sy - sz),
-     czx = load_vb(U, g, idx - sz - sx);
-  // E_x: (a,b) = (y,z);  E_y: (z,x);  E_z: (x,y);   args: cells (0,0), (-a,0), (0,-b), (-a,-b)
-  ct_one<0>(F, E, g, idx, c, cy, cz, cyz);
-  ct_one<1>(F, E, g, idx, c, cz, cx, czx);
-  ct_one<2>(F, E, g, idx, c, cx, cy, cxy);
+  ct_one<0>(F, Er, E, g, idx);
+  ct_one<1>(F, Er, E, g, idx);
+  ct_one<2>(F, Er, E, g, idx);
 }
 
 // ---------------------------------------------------------------------------------------
-// a4 / a8: update (O7).  Uout = Ubase - dts/Delta * flux differences (x, then y, then z);
+// a4 / a8: update (O7).  U_out = U^n - dts/Delta * flux differences (x, then y, then z);
 // face B from the edge fields.  One thread per index of [lo, hi+1]; cells are updated for
 // indices <= hi in all axes, the lower a-face where the two transverse indices are <= hi.
 // dts = scale * sc->dt (scale 1/2 for the half step, G8).
+// HALF = true: the result is stored in primitive form (rho, v, P, face B; see load_prim_half)
+// together with its reference field (Eq. 18); the thread then also needs its three UPPER faces
+// for the cell-centred field (Eq. 13), which it updates itself (same expression, same bits as the
+// owner of that face stores).
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_update(State8 Ubase, State8 Uout, Flux21 F, Edge3 E, Geo g,
-                                                Box box, const Scalars *sc, double scale) {
+template <int A>
+__device__ __forceinline__ double face_update(const State8 &U, const Edge3 &E, const Geo &g, long long idx,
+                                              const double dtd[3]) {  // Eq. 20-22 / 30-32
+  constexpr int B = (A + 1) % 3, C = (A + 2) % 3;
+  return __ldg(U.f[F_BX + A] + idx) + dtd[C] * (__ldg(E.f[B] + idx + g.s[C]) - __ldg(E.f[B] + idx)) -
+         dtd[B] * (__ldg(E.f[C] + idx + g.s[B]) - __ldg(E.f[C] + idx));
+}
+
+template <bool HALF>
+__global__ void __launch_bounds__(256) k_update(State8 Ubase, State8 Uout, Flux21 F, Edge3 E, Edge3 Er,
+                                                Geo g, Box box, const Scalars *sc, double scale) {
   const int lx = box.hi[0] - box.lo[0] + 2, ly = box.hi[1] - box.lo[1] + 2;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= lx * ly) return;
@@ -266,7 +272,11 @@ __global__ void __launch_bounds__(256) k_update(State8 Ubase, State8 Uout, Flux2
   const double dts = scale * sc->dt;
   double dtd[3];
 #pragma unroll
-  for (int a = 0; a < 3; a++) dtd[a] = dts / g.d[a];
+  for (int a = 0; a < 3; a++) dtd[a] = dts * (double)g.n[a];  // 1/Delta_a = n_a exactly
+  double Bl[3];
+  Bl[0] = (iny && inz) ? face_update<0>(Ubase, E, g, idx, dtd) : 0.0;
+  Bl[1] = (inz && inx) ? face_update<1>(Ubase, E, g, idx, dtd) : 0.0;
+  Bl[2] = (inx && iny) ? face_update<2>(Ubase, E, g, idx, dtd) : 0.0;
   if (inx && iny && inz) {
     double rho = Ubase.f[F_RHO][idx], En = Ubase.f[F_E][idx];
     double m[3] = {Ubase.f[F_MX][idx], Ubase.f[F_MY][idx], Ubase.f[F_MZ][idx]};
@@ -279,19 +289,41 @@ __global__ void __launch_bounds__(256) k_update(State8 Ubase, State8 Uout, Flux2
       m[(a + 2) % 3] -= dtd[a] * (__ldg(F.f[a][3] + up) - __ldg(F.f[a][3] + idx));
       En -= dtd[a] * (__ldg(F.f[a][4] + up) - __ldg(F.f[a][4] + idx));
     }
-    Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = m[0]; Uout.f[F_MY][idx] = m[1];
-    Uout.f[F_MZ][idx] = m[2]; Uout.f[F_E][idx] = En;
-  }
-  const bool in[3] = {inx, iny, inz};
+    if (HALF) {
+      Prim p;
+      p.rho = rho; p.ir = rcp(rho);
+      p.B[0] = 0.5 * (Bl[0] + face_update<0>(Ubase, E, g, idx + g.s[0], dtd));
+      p.B[1] = 0.5 * (Bl[1] + face_update<1>(Ubase, E, g, idx + g.s[1], dtd));
+      p.B[2] = 0.5 * (Bl[2] + face_update<2>(Ubase, E, g, idx + g.s[2], dtd));
 #pragma unroll
-  for (int a = 0; a < 3; a++) {  // Eq. 20-22 / 30-32
-    const int b = (a + 1) % 3, c = (a + 2) % 3;
-    if (in[b] && in[c]) {
-      Uout.f[F_BX + a][idx] = Ubase.f[F_BX + a][idx] +
-                              dtd[c] * (__ldg(E.f[b] + idx + g.s[c]) - __ldg(E.f[b] + idx)) -
-                              dtd[b] * (__ldg(E.f[c] + idx + g.s[b]) - __ldg(E.f[c] + idx));
+      for (int a = 0; a < 3; a++) p.v[a] = m[a] * p.ir;
+      p.P = pressure(g.gamma - 1.0, rho, p.v, En, p.B);
+      Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = p.v[0]; Uout.f[F_MY][idx] = p.v[1];
+      Uout.f[F_MZ][idx] = p.v[2]; Uout.f[F_E][idx] = p.P;
+      store_eref(Er, idx, p);
+    } else {
+      Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = m[0]; Uout.f[F_MY][idx] = m[1];
+      Uout.f[F_MZ][idx] = m[2]; Uout.f[F_E][idx] = En;
     }
   }
+  if (iny && inz) Uout.f[F_BX][idx] = Bl[0];
+  if (inz && inx) Uout.f[F_BY][idx] = Bl[1];
+  if (inx && iny) Uout.f[F_BZ][idx] = Bl[2];
+}
+
+// mhd_get_half_state: primitive half state -> conserved variables of the ABI
+__global__ void k_half_to_cons(State8 Wh, State8 Out, Geo g, Box box) {
+  const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= lx * ly) return;
+  int i = box.lo[0] + t % lx, j = box.lo[1] + t / lx, k = box.lo[2] + blockIdx.y;
+  long long idx = cell_index(g, i, j, k);
+  Prim p = load_prim_half(Wh, g, idx);
+  double v2 = p.v[0] * p.v[0] + p.v[1] * p.v[1] + p.v[2] * p.v[2];
+  double b2 = p.B[0] * p.B[0] + p.B[1] * p.B[1] + p.B[2] * p.B[2];
+  Out.f[F_RHO][idx] = p.rho;
+  Out.f[F_MX][idx] = p.rho * p.v[0]; Out.f[F_MY][idx] = p.rho * p.v[1]; Out.f[F_MZ][idx] = p.rho * p.v[2];
+  Out.f[F_E][idx] = p.P * g.gm1inv + 0.5 * p.rho * v2 + 0.5 * b2;
 }
 
 // max |div B| over the active cells (diagnostic)
@@ -342,7 +374,7 @@ __global__ void __launch_bounds__(MHD_BX, MHD_MINB_FX) k_flux_x(State8 Uh, Flux2
   double bn0 = 0.0;
   W7 W0;
   if (c <= cmax + R) {
-    Prim p = load_prim(Uh, g, row + c);
+    Prim p = load_prim_half(Uh, g, row + c);
     W0 = to_W<0>(p, bn0);
     sW[0][t + R] = W0.rho; sW[1][t + R] = W0.u; sW[2][t + R] = W0.v; sW[3][t + R] = W0.w;
     sW[4][t + R] = W0.P; sW[5][t + R] = W0.by; sW[6][t + R] = W0.bz;
@@ -352,7 +384,7 @@ __global__ void __launch_bounds__(MHD_BX, MHD_MINB_FX) k_flux_x(State8 Uh, Flux2
     int ch = cbase - R + slot;
     if (ch <= cmax + R) {
       double bnh;
-      Prim p = load_prim(Uh, g, row + ch);
+      Prim p = load_prim_half(Uh, g, row + ch);
       W7 Wh = to_W<0>(p, bnh);
       sW[0][slot] = Wh.rho; sW[1][slot] = Wh.u; sW[2][slot] = Wh.v; sW[3][slot] = Wh.w;
       sW[4][slot] = Wh.P; sW[5][slot] = Wh.by; sW[6][slot] = Wh.bz;
@@ -379,7 +411,7 @@ __global__ void __launch_bounds__(MHD_BX, MHD_MINB_FX) k_flux_x(State8 Uh, Flux2
     W7 WL;
     WL.rho = sH[0][t - 1]; WL.u = sH[1][t - 1]; WL.v = sH[2][t - 1]; WL.w = sH[3][t - 1];
     WL.P = sH[4][t - 1]; WL.by = sH[5][t - 1]; WL.bz = sH[6][t - 1];
-    F7 f = hlld(g.gamma, WL, lo, __ldg(Uh.f[F_BX] + row + c));
+    F7 f = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX] + row + c));
     store_flux<0>(F, row + c, f);
   }
 }
@@ -403,7 +435,7 @@ __global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux
   // window centred on cell f0-2 (slot 0 is never used): the loop below first shifts it
 #pragma unroll
   for (int s = 1; s < 2 * R + 1; s++) {
-    Prim p = load_prim(Uh, g, idx + (long long)(s - R - 2) * sA);
+    Prim p = load_prim_half(Uh, g, idx + (long long)(s - R - 2) * sA);
     win[s] = to_W<A>(p, bnc[s]);
   }
   win[0] = win[1]; bnc[0] = bnc[1];
@@ -416,12 +448,12 @@ __global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux
 #pragma unroll
     for (int s = 0; s < 2 * R; s++) { win[s] = win[s + 1]; bnc[s] = bnc[s + 1]; }
     {
-      Prim p = load_prim(Uh, g, idx + (long long)R * sA);
+      Prim p = load_prim_half(Uh, g, idx + (long long)R * sA);
       win[2 * R] = to_W<A>(p, bnc[2 * R]);
     }
     reconstruct<R>(g.gamma, win, bnc[R], lo, hi);
     if (f >= f0) {
-      F7 fl = hlld(g.gamma, WL, lo, __ldg(Uh.f[F_BX + A] + idx));
+      F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX + A] + idx));
       store_flux<A>(F, idx, fl);
     }
     WL = hi;

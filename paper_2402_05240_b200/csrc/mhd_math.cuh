@@ -1,0 +1,60 @@
+// mhd_math.cuh -- fp64 reciprocal, reciprocal square root and square root for the VL+CT kernels.
+//
+// nvcc's IEEE `/` and sqrt() expand to a MUFU seed, Newton steps, a range test and a call to a
+// slow path for denormal / huge operands: ~10 fp64-pipe instructions plus ~8 moves, compares and
+// branch bookkeeping each, and the step executes ~110 of them per cell.  Every operand here is a
+// physical quantity of ordinary magnitude (densities, speeds, pressures; never denormal, never
+// near overflow), so the slow path is dead weight.  These versions take the same hardware seed
+// (MUFU.RCP64H / MUFU.RSQ64H through PTX rcp.approx / rsqrt.approx, relative error < 2^-22) and
+// two Newton steps in fp64 FMAs (error -> 2^-44 -> rounding level).  The results are within 1 ulp
+// of the correctly rounded value: this is full fp64 precision, not -use_fast_math (which would
+// not touch fp64 anyway); the parity tolerance (1e-12) is four orders of magnitude looser.
+// Not valid for 0, denormal, infinite or NaN operands beyond what is noted per function.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mhd {
+
+// 1/x for normal x.
+__device__ __forceinline__ double rcp(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = __fma_rn(-x, y, 1.0);
+  y = __fma_rn(y, e, y);
+  e = __fma_rn(-x, y, 1.0);
+  y = __fma_rn(y, e, y);
+  return y;
+}
+
+// 1/sqrt(x) for normal x > 0.
+__device__ __forceinline__ double rsqrt_(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double h = 0.5 * x;
+  double e = __fma_rn(-h * y, y, 0.5);   // 1/2 - x y^2 / 2
+  y = __fma_rn(y, e, y);
+  e = __fma_rn(-h * y, y, 0.5);
+  y = __fma_rn(y, e, y);
+  return y;
+}
+
+// sqrt(x) for normal x > 0, and exactly 0 for x == 0 (x < 0 is the caller's bug).  Branch-free:
+// for x == 0 the seed is +inf and the NaN that follows is discarded by the final select.
+__device__ __forceinline__ double sqrt_(double x) {
+  double y = rsqrt_(x);
+  double s = x * y;
+  double r = __fma_rn(-s, s, x);  // residual x - s^2
+  s = __fma_rn(r, 0.5 * y, s);
+  return (x == 0.0) ? 0.0 : s;
+}
+
+// sqrt(x) and 1/sqrt(x) together, x > 0.
+__device__ __forceinline__ void sqrt_rsqrt(double x, double &s, double &is) {
+  double y = rsqrt_(x);
+  double t = x * y;
+  double r = __fma_rn(-t, t, x);
+  s = __fma_rn(r, 0.5 * y, t);
+  is = y;
+}
+
+}  // namespace mhd

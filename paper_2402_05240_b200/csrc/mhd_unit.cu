@@ -26,7 +26,8 @@ __global__ void k_unit_hlld(int n, double gamma, const double *WL, const double 
                             const double *bx, double *F) {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
-  F7 f = hlld(gamma, load_W(WL + 7 * t), load_W(WR + 7 * t), bx[t]);
+  W7 L = load_W(WL + 7 * t), R = load_W(WR + 7 * t);
+  F7 f = hlld(gamma, 1.0 / (gamma - 1.0), L, R, rcp(L.rho), rcp(R.rho), bx[t]);
   double *o = F + 7 * t;
   o[0] = f.m; o[1] = f.mn; o[2] = f.mt1; o[3] = f.mt2; o[4] = f.e; o[5] = f.by; o[6] = f.bz;
 }
@@ -49,6 +50,12 @@ __global__ void k_unit_ct(int n, const double *in, double *out) {
   if (t >= n) return;
   const double *p = in + 12 * t;
   out[t] = ct_edge(p[0], p[1], p[2], p[3], p[4], p[5], p[6], p[7], p[8], p[9], p[10], p[11]);
+}
+
+__global__ void k_unit_math(int n, int op, const double *x, double *y) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  y[t] = (op == 0) ? rcp(x[t]) : ((op == 1) ? rsqrt_(x[t]) : sqrt_(x[t]));
 }
 
 struct DevBuf {
@@ -95,5 +102,16 @@ extern "C" int mhd_unit_ct_edge(int n, const double *in12, double *out) {
   if (!a.up(in12, 12 * (size_t)n)) return MHD_ERR_CUDA;
   k_unit_ct<<<(n + 127) / 128, 128>>>(n, a.p, b.p);
   if (cudaGetLastError() != cudaSuccess || !b.down(out, n)) return MHD_ERR_CUDA;
+  return MHD_OK;
+}
+
+extern "C" int mhd_unit_math(int n, int op, const double *x, double *y) {
+  if (n < 0 || op < 0 || op > 2 || !x || !y) return MHD_ERR_ARG;
+  if (n == 0) return MHD_OK;
+  DevBuf a, b;
+  if (!a.alloc(n) || !b.alloc(n)) return MHD_ERR_NOMEM;
+  if (!a.up(x, n)) return MHD_ERR_CUDA;
+  k_unit_math<<<(n + 127) / 128, 128>>>(n, op, a.p, b.p);
+  if (cudaGetLastError() != cudaSuccess || !b.down(y, n)) return MHD_ERR_CUDA;
   return MHD_OK;
 }

@@ -57,12 +57,13 @@ def _load():
     L.mhd_unit_hlld.argtypes = [ctypes.c_int, ctypes.c_double, _dp, _dp, _dp, _dp]
     L.mhd_unit_reconstruct.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_int, _dp, _dp, _dp, _dp]
     L.mhd_unit_ct_edge.argtypes = [ctypes.c_int, _dp, _dp]
+    L.mhd_unit_math.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp]
     L.mhd_launch_count.restype = ctypes.c_longlong
     L.mhd_last_error.restype = ctypes.c_char_p
     for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_stream", "mhd_set_state",
                  "mhd_set_state_device", "mhd_compute_dt", "mhd_step", "mhd_advance", "mhd_get_state",
                  "mhd_get_state_device", "mhd_get_half_state", "mhd_max_divb", "mhd_synchronize",
-                 "mhd_finalize", "mhd_get_flux", "mhd_unit_hlld", "mhd_unit_reconstruct", "mhd_unit_ct_edge"):
+                 "mhd_finalize", "mhd_get_flux", "mhd_unit_hlld", "mhd_unit_reconstruct", "mhd_unit_ct_edge", "mhd_unit_math"):
         getattr(L, name).restype = ctypes.c_int
     return L
 
@@ -121,6 +122,14 @@ def unit_ct_edge(in12):
     out = np.empty(in12.shape[0])
     _check(_lib.mhd_unit_ct_edge(in12.shape[0], _hp(in12), _hp(out)))
     return out
+
+
+def unit_math(op, x):
+    """The kernels' rcp (op 0), rsqrt (op 1), sqrt (op 2) on the device."""
+    x = np.ascontiguousarray(x, dtype=np.float64).reshape(-1)
+    y = np.empty_like(x)
+    _check(_lib.mhd_unit_math(x.shape[0], int(op), _hp(x), _hp(y)))
+    return y
 
 
 class Mhd:
