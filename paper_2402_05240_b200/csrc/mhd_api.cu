@@ -121,9 +121,9 @@ int launch_corrector_fluxes() {
   // faces 0..n along the sweep, transverse -1..n (what CT and the final update need)
   {
     Box fb = make_box(0, n0, -1, n1, -1, n2);
-    int ncell = n0 + 2;  // cells -1..n
-    dim3 grid((ncell - 1 + (MHD_BX - 1) - 1) / (MHD_BX - 1), n1 + 2, n2 + 2);
-    k_flux_x<R><<<grid, MHD_BX, 0, C.stream>>>(C.Uh, C.F, g, fb);
+    int nwx = (n0 + 1 + 30) / 31;  // warps per pencil: 31 faces each, faces 0..n0
+    long long nw = (long long)nwx * (n1 + 2) * (n2 + 2);
+    k_flux_x<R><<<grid1(nw, 4), 128, 0, C.stream>>>(C.Uh, C.F, g, fb, nwx);
     LAUNCH_CHECK("k_flux_x");
   }
   {

@@ -43,7 +43,8 @@ __device__ __forceinline__ double fast_speed_sq(double gamma, double irho, doubl
 struct HlldSide {
   double rho, u, v, w, by, bz;        // primitive inputs
   double pT, e;                       // total pressure, total energy density
-  double rhos, vs, ws, bys, bzs, es;  // single-star state
+  double rhos, vs, ws, bys, bzs;      // single-star state (its energy is formed for one side only)
+  double Su, iSSm;                    // S - u, 1 / (S - S_M)
 };
 
 __device__ __forceinline__ void hlld_side_init(HlldSide &s, const W7 &W, double bx, double gm1inv) {
@@ -88,9 +89,7 @@ __device__ __forceinline__ void hlld_star(HlldSide &s, double S, double SM, doub
     s.bzs = s.bz * fb;
   }
   s.rhos = s.rho * (Su * iSSm);
-  double vb = s.u * bx + s.v * s.by + s.w * s.bz;
-  double vbs = SM * bx + s.vs * s.bys + s.ws * s.bzs;
-  s.es = (Su * s.e - s.pT * s.u + pTs * SM + bx * (vb - vbs)) * iSSm;
+  s.Su = Su; s.iSSm = iSSm;
 }
 
 // irL, irR = 1/rho of the two states (the callers have them or form them once)
@@ -131,8 +130,12 @@ __device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, co
   a.rho = left ? L.rho : R.rho; a.u = left ? L.u : R.u; a.v = left ? L.v : R.v; a.w = left ? L.w : R.w;
   a.by = left ? L.by : R.by; a.bz = left ? L.bz : R.bz; a.pT = left ? L.pT : R.pT; a.e = left ? L.e : R.e;
   a.rhos = left ? L.rhos : R.rhos; a.vs = left ? L.vs : R.vs; a.ws = left ? L.ws : R.ws;
-  a.bys = left ? L.bys : R.bys; a.bzs = left ? L.bzs : R.bzs; a.es = left ? L.es : R.es;
+  a.bys = left ? L.bys : R.bys; a.bzs = left ? L.bzs : R.bzs;
+  a.Su = left ? L.Su : R.Su; a.iSSm = left ? L.iSSm : R.iSSm;
   const double S = left ? SL : SR;
+  const double vb = a.u * bx + a.v * a.by + a.w * a.bz;
+  const double vbs = SM * bx + a.vs * a.bys + a.ws * a.bzs;
+  const double es = (a.Su * a.e - a.pT * a.u + pTs * SM + bx * (vb - vbs)) * a.iSSm;  // M&K Eq. 48
   F7 F = phys_flux(a, bx);
   const double Usmt1 = a.rhos * a.vs, Usmt2 = a.rhos * a.ws;
   // F*_a = F_a + S_a (U*_a - U_a)
@@ -140,7 +143,7 @@ __device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, co
   F.mn += S * (a.rhos * SM - a.rho * a.u);
   F.mt1 += S * (Usmt1 - a.rho * a.v);
   F.mt2 += S * (Usmt2 - a.rho * a.w);
-  F.e += S * (a.es - a.e);
+  F.e += S * (es - a.e);
   F.by += S * (a.bys - a.by);
   F.bz += S * (a.bzs - a.bz);
   if (dbl) {
@@ -153,13 +156,12 @@ __device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, co
     double byss = (rL * R.bys + rR * L.bys + rL * rR * (R.vs - L.vs) * sgn) * inv;
     double bzss = (rL * R.bzs + rR * L.bzs + rL * rR * (R.ws - L.ws) * sgn) * inv;
     double vbss = SM * bx + vss * byss + wss * bzss;
-    double vbs = SM * bx + a.vs * a.bys + a.ws * a.bzs;
     double r = left ? -rL : rR;
-    double ess = a.es + r * (vbs - vbss) * sgn;
+    double ess = es + r * (vbs - vbss) * sgn;
     // F**_a = F*_a + S*_a (U**_a - U*_a); rho** = rho*, u** = S_M
     F.mt1 += Ss * (a.rhos * vss - Usmt1);
     F.mt2 += Ss * (a.rhos * wss - Usmt2);
-    F.e += Ss * (ess - a.es);
+    F.e += Ss * (ess - es);
     F.by += Ss * (byss - a.bys);
     F.bz += Ss * (bzss - a.bzs);
     // mass and normal momentum: U** - U* = 0 exactly
@@ -279,7 +281,7 @@ __device__ __forceinline__ W7 eig_right(const Eig &e, const C7 &c) {
 // PLMC, Eq. 23-28 (reading O8).  Out: Wlo = W_{R,i-1/2}, Whi = W_{L,i+1/2}.
 // ---------------------------------------------------------------------------------------
 __device__ __forceinline__ double vl_slope(double dl, double dr) {  // Eq. 26 (G10)
-  return (dl * dr > 0.0) ? 2.0 * dl * dr / (dl + dr) : 0.0;
+  return (dl * dr > 0.0) ? 2.0 * dl * dr * rcp(dl + dr) : 0.0;
 }
 
 __device__ __forceinline__ double plm_limit(double aL, double aR, double aC, double aVL) {  // Eq. 27
@@ -294,13 +296,18 @@ __device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, c
                                      double bx0, W7 &Wlo, W7 &Whi) {
   Eig e;
   eig_setup(e, gamma, W0, bx0);
-  W7 dL, dR, dC, dV;
+  W7 dL, dR, dV;
 #define MHD_D4(f)                                   \
   dL.f = W0.f - Wm.f; dR.f = Wp.f - W0.f;           \
-  dC.f = (Wp.f - Wm.f) / 2.0; dV.f = vl_slope(dL.f, dR.f);
+  dV.f = vl_slope(dL.f, dR.f);
   MHD_D4(rho) MHD_D4(u) MHD_D4(v) MHD_D4(w) MHD_D4(P) MHD_D4(by) MHD_D4(bz)
 #undef MHD_D4
-  C7 aL = eig_left(e, dL), aR = eig_left(e, dR), aC = eig_left(e, dC), aV = eig_left(e, dV);
+  // L is linear and dC = (dL + dR)/2, so the centred amplitudes are the mean of the one-sided ones
+  C7 aL = eig_left(e, dL), aR = eig_left(e, dR), aV = eig_left(e, dV);
+  C7 aC;
+  aC.c0 = 0.5 * (aL.c0 + aR.c0); aC.c1 = 0.5 * (aL.c1 + aR.c1); aC.c2 = 0.5 * (aL.c2 + aR.c2);
+  aC.c3 = 0.5 * (aL.c3 + aR.c3); aC.c4 = 0.5 * (aL.c4 + aR.c4); aC.c5 = 0.5 * (aL.c5 + aR.c5);
+  aC.c6 = 0.5 * (aL.c6 + aR.c6);
   C7 am;
   am.c0 = plm_limit(aL.c0, aR.c0, aC.c0, aV.c0);
   am.c1 = plm_limit(aL.c1, aR.c1, aC.c1, aV.c1);
@@ -332,7 +339,7 @@ __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, doub
     double Dlim = 0.0;
     if (s != 0.0 && s == sgn3(Dj) && s == sgn3(Dj1))
       Dlim = s * fmin(fmin(C * fabs(Dj), C * fabs(Dj1)), fabs(Df));
-    qf = 0.5 * (qb + qc) - Dlim / 6.0;
+    qf = 0.5 * (qb + qc) - Dlim * (1.0 / 6.0);
   }
   return qf;
 }
@@ -359,7 +366,7 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
     double s = sgn3(Df);
     if (s != 0.0 && s == sgn3(Dm1) && s == sgn3(D0) && s == sgn3(Dp1))
       Dlim = s * fmin(fmin(C * fabs(Dm1), C * fabs(D0)), fmin(C * fabs(Dp1), fabs(Df)));
-    if (fabs(Df) > tau) r = Dlim / Df;
+    if (fabs(Df) > tau) r = Dlim * rcp(Df);
     if (r <= 1.0 - 1e-12) { qm = qi - r * dm; qp = qi + r * dp; }
   } else {
     if (fabs(dm) >= 2.0 * fabs(dp)) qm = qi - 2.0 * dp;

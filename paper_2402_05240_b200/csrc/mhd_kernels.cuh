@@ -358,61 +358,45 @@ __device__ __forceinline__ void reconstruct(double gamma, const W7 *win, double 
   else ppmc(gamma, win[0], win[1], win[2], win[3], win[4], bn0, lo, hi);      // O10
 }
 
-// x sweep: one thread per cell of an x pencil; the stencil and the hand-over of W_L go
-// through shared memory.  Block b owns cells c0 + b*(BX-1) + [0, BX) and faces 1..BX-1 of them.
-#define MHD_BX 128
+// x sweep: one WARP per 31 consecutive faces of an x pencil.  Lane l reconstructs cell c0 + l
+// (its stencil comes straight from global memory / L1: neighbouring lanes read the same lines);
+// the upper-face state W_{L,i+1/2} is handed to lane l+1 by warp shuffle, lanes 1..31 solve the
+// Riemann problem on their lower face.  No shared memory, no block barrier; consecutive warps
+// overlap by one cell (1/31 of the reconstructions are done twice).
+__device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+
 template <int R>
-__global__ void __launch_bounds__(MHD_BX, MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb) {
-  __shared__ double sW[7][MHD_BX + 2 * R + 1];
-  __shared__ double sH[7][MHD_BX];
-  const int t = threadIdx.x;
-  const int cbase = fb.lo[0] - 1 + blockIdx.x * (MHD_BX - 1);
-  const int c = cbase + t;
-  const int j = fb.lo[1] + blockIdx.y, k = fb.lo[2] + blockIdx.z;
-  const int cmax = fb.hi[0];  // last cell to reconstruct (= last face index)
-  const long long row = cell_index(g, 0, j, k);
-  double bn0 = 0.0;
-  W7 W0;
-  if (c <= cmax + R) {
-    Prim p = load_prim_half(Uh, g, row + c);
-    W0 = to_W<0>(p, bn0);
-    sW[0][t + R] = W0.rho; sW[1][t + R] = W0.u; sW[2][t + R] = W0.v; sW[3][t + R] = W0.w;
-    sW[4][t + R] = W0.P; sW[5][t + R] = W0.by; sW[6][t + R] = W0.bz;
-  }
-  if (R > 0 && t < 2 * R) {  // halo: R cells below the block, R above
-    int slot = (t < R) ? t : MHD_BX + t;
-    int ch = cbase - R + slot;
-    if (ch <= cmax + R) {
-      double bnh;
-      Prim p = load_prim_half(Uh, g, row + ch);
-      W7 Wh = to_W<0>(p, bnh);
-      sW[0][slot] = Wh.rho; sW[1][slot] = Wh.u; sW[2][slot] = Wh.v; sW[3][slot] = Wh.w;
-      sW[4][slot] = Wh.P; sW[5][slot] = Wh.by; sW[6][slot] = Wh.bz;
-    }
-  }
-  __syncthreads();
-  const bool active = (c <= cmax);
+__global__ void __launch_bounds__(128, MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb, int nwx) {
+  const int lane = threadIdx.x & 31;
+  const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int ly = fb.hi[1] - fb.lo[1] + 1, lz = fb.hi[2] - fb.lo[2] + 1;
+  if (wid >= (long long)nwx * ly * lz) return;  // whole warps only
+  const int wx = (int)(wid % nwx);
+  const long long row_id = wid / nwx;
+  const int j = fb.lo[1] + (int)(row_id % ly), k = fb.lo[2] + (int)(row_id / ly);
+  const int c = fb.lo[0] - 1 + wx * 31 + lane;  // cell of this lane
+  const bool active = (c <= fb.hi[0]);          // cells lo-1 .. hi are reconstructed
+  const long long idx = cell_index(g, c, j, k);
   W7 lo, hi;
   if (active) {
     W7 win[2 * R + 1];
+    double bnc[2 * R + 1];
 #pragma unroll
     for (int s = 0; s < 2 * R + 1; s++) {
-      if (s == R) { win[s] = W0; continue; }
-      win[s].rho = sW[0][t + s]; win[s].u = sW[1][t + s]; win[s].v = sW[2][t + s];
-      win[s].w = sW[3][t + s]; win[s].P = sW[4][t + s]; win[s].by = sW[5][t + s];
-      win[s].bz = sW[6][t + s];
+      Prim p = load_prim_half(Uh, g, idx + (s - R));
+      win[s] = to_W<0>(p, bnc[s]);
     }
-    reconstruct<R>(g.gamma, win, bn0, lo, hi);
-    sH[0][t] = hi.rho; sH[1][t] = hi.u; sH[2][t] = hi.v; sH[3][t] = hi.w; sH[4][t] = hi.P;
-    sH[5][t] = hi.by; sH[6][t] = hi.bz;
+    reconstruct<R>(g.gamma, win, bnc[R], lo, hi);
+  } else {
+    hi.rho = hi.u = hi.v = hi.w = hi.P = hi.by = hi.bz = 0.0;
+    lo = hi;
   }
-  __syncthreads();
-  if (active && t >= 1) {
-    W7 WL;
-    WL.rho = sH[0][t - 1]; WL.u = sH[1][t - 1]; WL.v = sH[2][t - 1]; WL.w = sH[3][t - 1];
-    WL.P = sH[4][t - 1]; WL.by = sH[5][t - 1]; WL.bz = sH[6][t - 1];
-    F7 f = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX] + row + c));
-    store_flux<0>(F, row + c, f);
+  W7 WL;
+  WL.rho = shfl_up1(hi.rho); WL.u = shfl_up1(hi.u); WL.v = shfl_up1(hi.v); WL.w = shfl_up1(hi.w);
+  WL.P = shfl_up1(hi.P); WL.by = shfl_up1(hi.by); WL.bz = shfl_up1(hi.bz);
+  if (active && lane >= 1) {
+    F7 f = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX] + idx));
+    store_flux<0>(F, idx, f);
   }
 }
 
