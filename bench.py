@@ -30,21 +30,27 @@ METRIC = "fp64 MHD cell updates/sec (VL+CT, HLLD, PLMC)"
 UNIT = "cell updates/s"
 CFL = 0.4
 
-# Algorithmic work per cell update: fp64 FLOPs (add/mul = 1, fma = 2)
-# executed per cell by each kernel as counted with ncu on the 256^3 workload, and the HBM
-# bytes each kernel must move per cell (compulsory reads + writes of its operands).
+# Algorithmic work per cell update: fp64 FLOPs (dadd + dmul + 2 dfma,
+# thread-level, predicated-on) executed per ACTIVE cell by each kernel as counted by ncu on the
+# 256^3 PLMC workload (profiles/r1_ncu_kernels.md), and the HBM bytes each kernel must move per
+# cell (compulsory reads + writes of its operand arrays, 8 B each).
 KERNEL_MODEL = {
-    #                      flop/cell  bytes/cell
-    "k_predictor_flux": (None, (8 + 21) * 8),
-    "k_flux_x": (None, (8 + 7) * 8),
-    "k_flux_march<1>": (None, (8 + 7) * 8),
-    "k_flux_march<2>": (None, (8 + 7) * 8),
-    "k_ct(predictor)": (None, (9 + 7 + 3) * 8),
-    "k_ct(corrector)": (None, (9 + 7 + 3) * 8),
-    "k_update(half)": (None, (8 + 15 + 3 + 8) * 8),
-    "k_update(full)": (None, (8 + 15 + 3 + 8) * 8),
-    "k_cfl": (None, 8 * 8),
+    #                         flop/cell  bytes/cell
+    "k_predictor_flux":      (1212, (8 + 21 + 3) * 8),       # U^n -> 21 fluxes + reference field
+    "k_ct(predictor)":       (81, (9 + 3 + 3) * 8),          # mass/magnetic fluxes + E_ref -> edge E
+    "k_update(half)":        (139, (8 + 15 + 3 + 8 + 3) * 8),  # U^n, hydro fluxes, edge E -> W^{n+1/2}, E_ref
+    "k_flux_x":              (913, (8 + 7) * 8),             # W^{n+1/2} -> 7 fluxes
+    "k_flux_march<1>":       (911, (8 + 7) * 8),
+    "k_flux_march<2>":       (898, (8 + 7) * 8),
+    "k_ct(corrector)":       (77, (9 + 3 + 3) * 8),
+    "k_update(full)+cfl":    (266, (8 + 15 + 3 + 8) * 8),    # U^n, hydro fluxes, edge E -> U^{n+1}; CFL rate
 }
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (GB) from the same ncu capture
+NCU_TRAFFIC_GB = {"k_predictor_flux": 4.69, "k_ct(predictor)": 2.16, "k_update(half)": 5.32, "k_flux_x": 2.07,
+                  "k_flux_march<1>": 2.13, "k_flux_march<2>": 2.13, "k_ct(corrector)": 2.09,
+                  "k_update(full)+cfl": 4.67}
+STEP_FLOP_PER_CELL = sum(v[0] for v in KERNEL_MODEL.values())     # 4497 (PLMC)
+STEP_BYTES_PER_CELL = sum(v[1] for v in KERNEL_MODEL.values())    # 1496 as materialised; floor 128
 
 
 def parse_args():
@@ -315,10 +321,15 @@ def run_b200(args):
         step_ms = sum(prof.values())
         top = max((k for k in prof if k in KERNEL_MODEL), key=lambda k: prof[k])
         flop_cell, byte_cell = KERNEL_MODEL[top]
+        if p.recon != 1:
+            flop_cell = None  # FLOP counts were taken on the PLMC build only
         t_top = prof[top] * 1e-3
+        traffic = NCU_TRAFFIC_GB.get(top) if (tuple(p.n) == (256, 256, 256) and p.recon == 1) else None
         roof = {"kernel": top, "kernel_ms": prof[top], "share_of_step": prof[top] / step_ms,
-                "traffic": None}
+                "traffic": traffic * 1e9 if traffic else None,
+                "traffic_source": "profiles/r1_ncu_kernels.md (ncu --set full, 256^3 PLMC)" if traffic else None}
         hbm_ach = byte_cell * nc / t_top / 1e9
+        roof["algorithmic_bytes_per_launch"] = byte_cell * nc
         if flop_cell is not None and flop_cell * nc / (fp64_tf * 1e12) > byte_cell * nc / (hbm_peak * 1e9):
             ach = flop_cell * nc / t_top / 1e12
             roof.update({"bound": "alu", "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s",
@@ -327,6 +338,19 @@ def run_b200(args):
         else:
             roof.update({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
                          "frac": hbm_ach / hbm_peak, "peak_source": hbm_src})
+            if flop_cell is not None:
+                roof["fp64_achieved_tflops"] = flop_cell * nc / t_top / 1e12
+        # whole-step roofline (north_star): the slower of counted FLOPs at the measured fp64 peak and
+        # the bytes the design moves at the measured HBM bandwidth; the 128 B/cell floor beside it
+        if p.recon == 1:
+            t_flop = STEP_FLOP_PER_CELL * nc / (fp64_tf * 1e12)
+            t_byte = STEP_BYTES_PER_CELL * nc / (hbm_peak * 1e9)
+            t_step = ms / args.steps * 1e-3 / 1.0
+            roof["step"] = {"flop_per_cell": STEP_FLOP_PER_CELL, "bytes_per_cell": STEP_BYTES_PER_CELL,
+                            "t_flop_ms": t_flop * 1e3, "t_bytes_ms": t_byte * 1e3,
+                            "frac_of_roofline": max(t_flop, t_byte) / t_step,
+                            "frac_of_128B_floor": (128.0 * nc / (hbm_peak * 1e9)) / t_step,
+                            "fp64_tflops_step": STEP_FLOP_PER_CELL * nc / t_step / 1e12}
         roof["kernels_ms"] = {k: round(v, 4) for k, v in prof.items()}
         roof["measured_here"] = {"fp64_tflops": fp64_tf, "copy_gbs": copy_gbs}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -23,9 +23,11 @@ struct Context {
   Flux21 F;
   Edge3 E;   // CT edge fields
   Edge3 Er;  // cell-centred reference field, Eq. 18
+  Edge3 Bnext;  // face arrays that receive B^{n+1}; swapped with U's after every step
   Scalars *sc = nullptr;
   cudaStream_t stream = 0;
   long long launches = 0;
+  bool rate_valid = false;  // sc->rate_bits holds the CFL rate of the current state
   // per-launch event timing (mhd_step_profile)
   int prof_n = -1;  // -1 = off, else number of launches recorded so far
   cudaEvent_t prof_ev[kMaxProf + 1];
@@ -81,7 +83,7 @@ bool make_geo(Geo &g, int nx, int ny, int nz, double gamma, int recon) {
   return true;
 }
 
-const int kNumArrays = 2 * NFIELD + 21 + 3 + 3;  // U, half state, fluxes, edge fields, reference field
+const int kNumArrays = 2 * NFIELD + 21 + 3 + 3 + 3;  // U, half state, fluxes, edge fields, reference field, B^{n+1}
 
 size_t array_bytes(const Geo &g) { return ((size_t)g.ntot * sizeof(double) + 255) / 256 * 256; }
 
@@ -192,18 +194,29 @@ int step_kernels() {
     k_ct<<<grid, 256, 0, C.stream>>>(C.F, C.Er, C.E, g, eb);
     LAUNCH_CHECK("k_ct(corrector)");
     dim3 gridu(grid1(plane, 256).x, g.n[2] + 1);
-    k_update<false><<<gridu, 256, 0, C.stream>>>(C.U, C.U, C.F, C.E, C.Er, g, ab, C.sc, 1.0);
-    LAUNCH_CHECK("k_update(full)");
+    // hydro fields in place; B^{n+1} goes to a second set of face arrays which then become the
+    // state's (pointer swap): a thread reads B^n on its upper faces, owned by other threads
+    State8 out = C.U;
+    for (int a = 0; a < 3; a++) out.f[F_BX + a] = C.Bnext.f[a];
+    k_update<false><<<gridu, 256, 0, C.stream>>>(C.U, out, C.F, C.E, C.Er, g, ab, C.sc, 1.0);
+    LAUNCH_CHECK("k_update(full)+cfl");
+    for (int a = 0; a < 3; a++) { C.Bnext.f[a] = C.U.f[F_BX + a]; C.U.f[F_BX + a] = out.f[F_BX + a]; }
+    C.rate_valid = true;
   }
   return MHD_OK;
 }
 
-int cfl_kernel() {
+// CFL rate of the current state into sc->rate_bits, unless the last full update left it there
+int ensure_rate() {
+  if (C.rate_valid) return MHD_OK;
   const Geo &g = C.g;
+  k_reset_rate<<<1, 1, 0, C.stream>>>(C.sc);
+  LAUNCH_CHECK("k_reset_rate");
   long long plane = (long long)g.n[0] * g.n[1];
   dim3 grid(grid1(plane, 256).x, g.n[2]);
   k_cfl<<<grid, 256, 0, C.stream>>>(C.U, g, C.sc);
   LAUNCH_CHECK("k_cfl");
+  C.rate_valid = true;
   return MHD_OK;
 }
 
@@ -231,7 +244,9 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
     for (int c = 0; c < 7; c++) { C.F.f[a][c] = (double *)p; p += ab; }
   for (int a = 0; a < 3; a++) { C.E.f[a] = (double *)p; p += ab; }
   for (int a = 0; a < 3; a++) { C.Er.f[a] = (double *)p; p += ab; }
+  for (int a = 0; a < 3; a++) { C.Bnext.f[a] = (double *)p; p += ab; }
   C.launches = 0;
+  C.rate_valid = false;
   C.inited = true;
   cudaError_t e = cudaMemsetAsync(C.base, 0, need, C.stream);
   if (e != cudaSuccess) { mhd_finalize(); return cuda_fail(e, "cudaMemsetAsync"); }
@@ -257,6 +272,7 @@ int set_state_from(const double *const src[NFIELD], bool host) {
     k_unpack<<<grid1(cnt, 256), 256, 0, C.stream>>>(C.U.f[f], dsrc, g, ex, ey, ez);
     LAUNCH_CHECK("k_unpack");
   }
+  C.rate_valid = false;
   return fill_ghosts(C.U);
 }
 
@@ -328,12 +344,10 @@ int mhd_set_state_device(const double *rho, const double *mx, const double *my, 
 int mhd_compute_dt(double cfl, double *dt) {
   if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
   if (!dt || !(cfl > 0.0)) return fail(MHD_ERR_ARG, "mhd_compute_dt: bad argument");
-  int rc = cfl_kernel();
+  int rc = ensure_rate();
   if (rc) return rc;
   Scalars h;
   CU(cudaMemcpyAsync(&h, C.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, C.stream));
-  k_reset_rate<<<1, 1, 0, C.stream>>>(C.sc);
-  LAUNCH_CHECK("k_reset_rate");
   CU(cudaStreamSynchronize(C.stream));
   double m;
   memcpy(&m, &h.rate_bits, sizeof(double));
@@ -361,7 +375,7 @@ int mhd_advance(int n_steps, double cfl, double *t_accum) {
     t0 = h.t_accum;
   }
   for (int s = 0; s < n_steps; s++) {
-    int rc = cfl_kernel();
+    int rc = ensure_rate();
     if (rc) return rc;
     k_finish_dt<<<1, 1, 0, C.stream>>>(C.sc, cfl);
     LAUNCH_CHECK("k_finish_dt");
@@ -452,12 +466,7 @@ int mhd_step_profile(double dt, int max_entries, double *ms, const char **names,
   LAUNCH_CHECK("k_set_dt");
   C.prof_n = 0;
   cudaEventRecord(C.prof_ev[0], C.stream);
-  int rc = cfl_kernel();
-  if (!rc) {
-    k_reset_rate<<<1, 1, 0, C.stream>>>(C.sc);
-    C.launches++;
-    rc = step_kernels();
-  }
+  int rc = step_kernels();
   int n = C.prof_n;
   C.prof_n = -1;
   cudaError_t e = cudaStreamSynchronize(C.stream);

@@ -161,7 +161,8 @@ __global__ void k_finish_dt(Scalars *sc, double cfl) {
   sc->rate_bits = 0ull;
 }
 
-__global__ void k_set_dt(Scalars *sc, double dt) { sc->dt = dt; }
+// dt given by the caller; re-arm the reduction (the full update accumulates the next rate)
+__global__ void k_set_dt(Scalars *sc, double dt) { sc->dt = dt; sc->rate_bits = 0ull; }
 
 // Eq. 18: cell-centred reference field E = -(v x B)
 __device__ __forceinline__ void store_eref(const Edge3 &Er, long long idx, const Prim &p) {
@@ -188,11 +189,19 @@ __device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const
   store_flux<A>(F, idx, f);
 }
 
+// minimum resident blocks per SM asked of ptxas (register caps), tuned on B200 at 256^3:
+// the fp64-bound kernels want warps (128 registers), the HBM-bound ones want loads in flight
+#ifndef MHD_MINB_UPD
+#define MHD_MINB_UPD 2
+#endif
+#ifndef MHD_MINB_CT
+#define MHD_MINB_CT 3
+#endif
 #ifndef MHD_MINB_PRED
-#define MHD_MINB_PRED 4
+#define MHD_MINB_PRED 5
 #endif
 #ifndef MHD_MINB_FX
-#define MHD_MINB_FX 4
+#define MHD_MINB_FX 5
 #endif
 #ifndef MHD_MINB_FM
 #define MHD_MINB_FM 4
@@ -231,7 +240,7 @@ __device__ __forceinline__ void ct_one(const Flux21 &F, const Edge3 &Er, const E
                         __ldg(er + idx - sb), __ldg(er + idx - sa - sb));
 }
 
-__global__ void __launch_bounds__(256) k_ct(Flux21 F, Edge3 Er, Edge3 E, Geo g, Box box) {
+__global__ void __launch_bounds__(256, MHD_MINB_CT) k_ct(Flux21 F, Edge3 Er, Edge3 E, Geo g, Box box) {
   const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= lx * ly) return;
@@ -261,13 +270,14 @@ __device__ __forceinline__ double face_update(const State8 &U, const Edge3 &E, c
 }
 
 template <bool HALF>
-__global__ void __launch_bounds__(256) k_update(State8 Ubase, State8 Uout, Flux21 F, Edge3 E, Edge3 Er,
-                                                Geo g, Box box, const Scalars *sc, double scale) {
+__global__ void __launch_bounds__(256, MHD_MINB_UPD) k_update(State8 Ubase, State8 Uout, Flux21 F, Edge3 E, Edge3 Er,
+                                                Geo g, Box box, Scalars *sc, double scale) {
   const int lx = box.hi[0] - box.lo[0] + 2, ly = box.hi[1] - box.lo[1] + 2;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= lx * ly) return;
+  const bool valid = t < lx * ly;
+  if (!valid) t = 0;
   int i = box.lo[0] + t % lx, j = box.lo[1] + t / lx, k = box.lo[2] + blockIdx.y;
-  const bool inx = i <= box.hi[0], iny = j <= box.hi[1], inz = k <= box.hi[2];
+  const bool inx = valid && i <= box.hi[0], iny = valid && j <= box.hi[1], inz = valid && k <= box.hi[2];
   long long idx = cell_index(g, i, j, k);
   const double dts = scale * sc->dt;
   double dtd[3];
@@ -277,6 +287,8 @@ __global__ void __launch_bounds__(256) k_update(State8 Ubase, State8 Uout, Flux2
   Bl[0] = (iny && inz) ? face_update<0>(Ubase, E, g, idx, dtd) : 0.0;
   Bl[1] = (inz && inx) ? face_update<1>(Ubase, E, g, idx, dtd) : 0.0;
   Bl[2] = (inx && iny) ? face_update<2>(Ubase, E, g, idx, dtd) : 0.0;
+  double rate = 0.0;
+  int bad = 0;
   if (inx && iny && inz) {
     double rho = Ubase.f[F_RHO][idx], En = Ubase.f[F_E][idx];
     double m[3] = {Ubase.f[F_MX][idx], Ubase.f[F_MY][idx], Ubase.f[F_MZ][idx]};
@@ -289,26 +301,31 @@ __global__ void __launch_bounds__(256) k_update(State8 Ubase, State8 Uout, Flux2
       m[(a + 2) % 3] -= dtd[a] * (__ldg(F.f[a][3] + up) - __ldg(F.f[a][3] + idx));
       En -= dtd[a] * (__ldg(F.f[a][4] + up) - __ldg(F.f[a][4] + idx));
     }
-    if (HALF) {
-      Prim p;
-      p.rho = rho; p.ir = rcp(rho);
-      p.B[0] = 0.5 * (Bl[0] + face_update<0>(Ubase, E, g, idx + g.s[0], dtd));
-      p.B[1] = 0.5 * (Bl[1] + face_update<1>(Ubase, E, g, idx + g.s[1], dtd));
-      p.B[2] = 0.5 * (Bl[2] + face_update<2>(Ubase, E, g, idx + g.s[2], dtd));
+    // primitives of the updated cell: the half step stores them; the full step needs them for the
+    // next step's CFL rate (Eq. 11), folded in here so that the state is not read once more
+    Prim p;
+    p.rho = rho; p.ir = rcp(rho);
+    p.B[0] = 0.5 * (Bl[0] + face_update<0>(Ubase, E, g, idx + g.s[0], dtd));
+    p.B[1] = 0.5 * (Bl[1] + face_update<1>(Ubase, E, g, idx + g.s[1], dtd));
+    p.B[2] = 0.5 * (Bl[2] + face_update<2>(Ubase, E, g, idx + g.s[2], dtd));
 #pragma unroll
-      for (int a = 0; a < 3; a++) p.v[a] = m[a] * p.ir;
-      p.P = pressure(g.gamma - 1.0, rho, p.v, En, p.B);
+    for (int a = 0; a < 3; a++) p.v[a] = m[a] * p.ir;
+    p.P = pressure(g.gamma - 1.0, rho, p.v, En, p.B);
+    if (HALF) {
       Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = p.v[0]; Uout.f[F_MY][idx] = p.v[1];
       Uout.f[F_MZ][idx] = p.v[2]; Uout.f[F_E][idx] = p.P;
       store_eref(Er, idx, p);
     } else {
       Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = m[0]; Uout.f[F_MY][idx] = m[1];
       Uout.f[F_MZ][idx] = m[2]; Uout.f[F_E][idx] = En;
+      rate = cell_rate(g, p, bad);
     }
   }
+  // the face arrays of Uout are never those of Ubase (the upper-face reads above would race)
   if (iny && inz) Uout.f[F_BX][idx] = Bl[0];
   if (inz && inx) Uout.f[F_BY][idx] = Bl[1];
   if (inx && iny) Uout.f[F_BZ][idx] = Bl[2];
+  if (!HALF) block_rate_reduce(rate, bad, sc);
 }
 
 // mhd_get_half_state: primitive half state -> conserved variables of the ABI
