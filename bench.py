@@ -41,14 +41,14 @@ KERNEL_MODEL = {
     "k_update(half)":        (139, (8 + 15 + 3 + 8 + 3) * 8),  # U^n, hydro fluxes, edge E -> W^{n+1/2}, E_ref
     "k_flux_x":              (913, (8 + 7) * 8),             # W^{n+1/2} -> 7 fluxes
     "k_flux_march<1>":       (911, (8 + 7) * 8),
-    "k_flux_march<2>":       (898, (8 + 7) * 8),
+    "k_flux_march<2>+update": (898 + 50, (8 + 3 + 5 + 10 + 5) * 8),  # + U^n, x/y hydro fluxes -> U^{n+1} hydro
     "k_ct(corrector)":       (77, (9 + 3 + 3) * 8),
-    "k_update(full)+cfl":    (266, (8 + 15 + 3 + 8) * 8),    # U^n, hydro fluxes, edge E -> U^{n+1}; CFL rate
+    "k_update(B)+cfl":       (216, (8 + 3 + 3) * 8),         # B^n, edge E -> B^{n+1}; U^{n+1} -> CFL rate
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (GB) from the same ncu capture
 NCU_TRAFFIC_GB = {"k_predictor_flux": 4.69, "k_ct(predictor)": 2.16, "k_update(half)": 5.32, "k_flux_x": 2.07,
-                  "k_flux_march<1>": 2.13, "k_flux_march<2>": 2.13, "k_ct(corrector)": 2.09,
-                  "k_update(full)+cfl": 4.67}
+                  "k_flux_march<1>": 2.13, "k_ct(corrector)": 2.09,
+                  }  # the z sweep and the B update changed after that capture: no entry (traffic null)
 STEP_FLOP_PER_CELL = sum(v[0] for v in KERNEL_MODEL.values())     # 4497 (PLMC)
 STEP_BYTES_PER_CELL = sum(v[1] for v in KERNEL_MODEL.values())    # 1496 as materialised; floor 128
 

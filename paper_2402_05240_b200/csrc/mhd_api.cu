@@ -136,7 +136,7 @@ int launch_corrector_fluxes() {
 #endif
     long long nt = (long long)(n0 + 2) * (n2 + 2);
     dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
-    k_flux_march<1, R><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J);
+    k_flux_march<1, R, false><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<1>");
   }
   {
@@ -144,8 +144,8 @@ int launch_corrector_fluxes() {
     int J = (n2 + 1 >= 64) ? 32 : ((n2 + 1 >= 16) ? 8 : 4);
     long long nt = (long long)(n0 + 2) * (n1 + 2);
     dim3 grid(grid1(nt, 128).x, (n2 + 1 + J - 1) / J);
-    k_flux_march<2, R><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J);
-    LAUNCH_CHECK("k_flux_march<2>");
+    k_flux_march<2, R, true><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
+    LAUNCH_CHECK("k_flux_march<2>+update");
   }
   return MHD_OK;
 }
@@ -199,7 +199,7 @@ int step_kernels() {
     State8 out = C.U;
     for (int a = 0; a < 3; a++) out.f[F_BX + a] = C.Bnext.f[a];
     k_update<false><<<gridu, 256, 0, C.stream>>>(C.U, out, C.F, C.E, C.Er, g, ab, C.sc, 1.0);
-    LAUNCH_CHECK("k_update(full)+cfl");
+    LAUNCH_CHECK("k_update(B)+cfl");
     for (int a = 0; a < 3; a++) { C.Bnext.f[a] = C.U.f[F_BX + a]; C.U.f[F_BX + a] = out.f[F_BX + a]; }
     C.rate_valid = true;
   }
@@ -430,6 +430,8 @@ int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *
 int mhd_get_flux(int axis, int comp, double *out) {
   if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
   if (axis < 0 || axis > 2 || comp < 0 || comp > 6 || !out) return fail(MHD_ERR_ARG, "mhd_get_flux: bad argument");
+  if (axis == 2 && comp >= 1 && comp <= 4)
+    return fail(MHD_ERR_ARG, "mhd_get_flux: the z momentum / energy fluxes are consumed in the z sweep, not stored");
   const Geo &g = C.g;
   long long cnt = (long long)g.n[0] * g.n[1] * g.n[2];
   double *stage = C.Uh.f[0];  // the half-step state is dead after the step

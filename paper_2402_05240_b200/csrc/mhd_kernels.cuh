@@ -253,7 +253,9 @@ __global__ void __launch_bounds__(256, MHD_MINB_CT) k_ct(Flux21 F, Edge3 Er, Edg
 
 // ---------------------------------------------------------------------------------------
 // a4 / a8: update (O7).  U_out = U^n - dts/Delta * flux differences (x, then y, then z);
-// face B from the edge fields.  One thread per index of [lo, hi+1]; cells are updated for
+// face B from the edge fields.  HALF = false: the hydro variables of U^{n+1} were already written by
+// the z sweep (k_flux_march<2,R,true>); this kernel updates the face field (Eq. 30-32) and forms the
+// CFL rate of the new state.  One thread per index of [lo, hi+1]; cells are updated for
 // indices <= hi in all axes, the lower a-face where the two transverse indices are <= hi.
 // dts = scale * sc->dt (scale 1/2 for the half step, G8).
 // HALF = true: the result is stored in primitive form (rho, v, P, face B; see load_prim_half)
@@ -292,14 +294,16 @@ __global__ void __launch_bounds__(256, MHD_MINB_UPD) k_update(State8 Ubase, Stat
   if (inx && iny && inz) {
     double rho = Ubase.f[F_RHO][idx], En = Ubase.f[F_E][idx];
     double m[3] = {Ubase.f[F_MX][idx], Ubase.f[F_MY][idx], Ubase.f[F_MZ][idx]};
+    if (HALF) {  // Eq. 19; in the full step the z sweep has already applied Eq. 29 to these five
 #pragma unroll
-    for (int a = 0; a < 3; a++) {
-      long long up = idx + g.s[a];
-      rho -= dtd[a] * (__ldg(F.f[a][0] + up) - __ldg(F.f[a][0] + idx));
-      m[a] -= dtd[a] * (__ldg(F.f[a][1] + up) - __ldg(F.f[a][1] + idx));
-      m[(a + 1) % 3] -= dtd[a] * (__ldg(F.f[a][2] + up) - __ldg(F.f[a][2] + idx));
-      m[(a + 2) % 3] -= dtd[a] * (__ldg(F.f[a][3] + up) - __ldg(F.f[a][3] + idx));
-      En -= dtd[a] * (__ldg(F.f[a][4] + up) - __ldg(F.f[a][4] + idx));
+      for (int a = 0; a < 3; a++) {
+        long long up = idx + g.s[a];
+        rho -= dtd[a] * (__ldg(F.f[a][0] + up) - __ldg(F.f[a][0] + idx));
+        m[a] -= dtd[a] * (__ldg(F.f[a][1] + up) - __ldg(F.f[a][1] + idx));
+        m[(a + 1) % 3] -= dtd[a] * (__ldg(F.f[a][2] + up) - __ldg(F.f[a][2] + idx));
+        m[(a + 2) % 3] -= dtd[a] * (__ldg(F.f[a][3] + up) - __ldg(F.f[a][3] + idx));
+        En -= dtd[a] * (__ldg(F.f[a][4] + up) - __ldg(F.f[a][4] + idx));
+      }
     }
     // primitives of the updated cell: the half step stores them; the full step needs them for the
     // next step's CFL rate (Eq. 11), folded in here so that the state is not read once more
@@ -316,8 +320,6 @@ __global__ void __launch_bounds__(256, MHD_MINB_UPD) k_update(State8 Ubase, Stat
       Uout.f[F_MZ][idx] = p.v[2]; Uout.f[F_E][idx] = p.P;
       store_eref(Er, idx, p);
     } else {
-      Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = m[0]; Uout.f[F_MY][idx] = m[1];
-      Uout.f[F_MZ][idx] = m[2]; Uout.f[F_E][idx] = En;
       rate = cell_rate(g, p, bad);
     }
   }
@@ -417,11 +419,30 @@ __global__ void __launch_bounds__(128, MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F
   }
 }
 
+// Asynchronous 8-byte global -> shared copies (LDGSTS): the operands of the fused hydro update are
+// fetched one marching iteration ahead into a per-thread column of shared memory, so their HBM
+// latency hides behind a whole reconstruction + Riemann solve at no cost in registers.
+__device__ __forceinline__ void cp_async8(double *smem, const double *gmem) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 // y / z sweep: a thread owns one x position (warps run along x, so every load and store is
 // coalesced) and marches along the sweep axis over a chunk of J faces with a rolling window
 // of 2R+1 primitive states in registers; each cell's primitives are formed once per chunk.
-template <int A, int R>
-__global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J) {
+//
+// UPDATE (z sweep only, the last of the three): the thread holds the z fluxes on both faces of cell
+// f-1, and the x and y fluxes are already in memory, so it applies Eq. 29 to the hydro variables of
+// that cell on the spot (U^n -> U^{n+1} in place; nothing else reads U^n's hydro fields any more).
+// The four momentum / energy z fluxes then never go to memory (the mass and magnetic fluxes still
+// do, for the CT kernel), and the full update that follows only has the face field left to do.
+// A chunk then also solves face f1+1 (its last cell needs it; 1/J more Riemann solves).
+template <int A, int R, bool UPDATE>
+__global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
+                                                                  State8 U, const Scalars *sc) {
+  static_assert(!UPDATE || A == 2, "the fused hydro update rides on the z sweep");
   constexpr int O = (A == 1) ? 2 : 1;  // the other transverse axis
   const int lx = fb.hi[0] - fb.lo[0] + 1, lo_ = fb.hi[O] - fb.lo[O] + 1;
   long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -429,8 +450,16 @@ __global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux
   const int i = fb.lo[0] + (int)(t % lx), o = fb.lo[O] + (int)(t / lx);
   const int f0 = fb.lo[A] + blockIdx.y * J;
   const int f1 = min(f0 + J - 1, fb.hi[A]);
+  const int fend = (UPDATE && f1 < fb.hi[A]) ? f1 + 1 : f1;
   const long long sA = g.s[A];
   long long idx = (A == 1) ? cell_index(g, i, f0, o) : cell_index(g, i, o, f0);  // cell f0
+  const bool upd_col = UPDATE && i >= 0 && i < g.n[0] && o >= 0 && o < g.n[O];  // an active column
+  double dtd[3] = {0.0, 0.0, 0.0};
+  if (UPDATE) {
+    const double dt = sc->dt;
+#pragma unroll
+    for (int a = 0; a < 3; a++) dtd[a] = dt * (double)g.n[a];
+  }
   W7 win[2 * R + 1];
   double bnc[2 * R + 1];
   // window centred on cell f0-2 (slot 0 is never used): the loop below first shifts it
@@ -441,11 +470,18 @@ __global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux
   }
   win[0] = win[1]; bnc[0] = bnc[1];
   W7 WL = win[1], lo, hi;
+  F7 fprev;
+  fprev.m = fprev.mn = fprev.mt1 = fprev.mt2 = fprev.e = fprev.by = fprev.bz = 0.0;
+  // staging column of this thread: slots 0..4 = U (rho, mx, my, mz, E) of the cell to update,
+  // 5 + 10 a + 2 q + {0, 1} = flux component q of sweep a (x, y) on its lower / upper face
+  __shared__ double stage[UPDATE ? 25 : 1][UPDATE ? 128 : 1];
+  const int tid = threadIdx.x;
+  const int last_cell = min(f1, g.n[A] - 1);
   idx -= sA;
   // One reconstruct() call site per kernel: iteration f0-1 only produces W_L of face f0; every
   // cell is then reconstructed by the same instruction sequence, so mirror-image cells give
   // mirror-image states bit for bit.
-  for (int f = f0 - 1; f <= f1; f++, idx += sA) {
+  for (int f = f0 - 1; f <= fend; f++, idx += sA) {
 #pragma unroll
     for (int s = 0; s < 2 * R; s++) { win[s] = win[s + 1]; bnc[s] = bnc[s + 1]; }
     {
@@ -455,7 +491,47 @@ __global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux
     reconstruct<R>(g.gamma, win, bnc[R], lo, hi);
     if (f >= f0) {
       F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX + A] + idx));
-      store_flux<A>(F, idx, fl);
+      if (!UPDATE) {
+        store_flux<A>(F, idx, fl);
+      } else {
+        if (f <= f1) { F.f[A][0][idx] = fl.m; F.f[A][5][idx] = fl.by; F.f[A][6][idx] = fl.bz; }
+        if (upd_col && f > f0 && f - 1 <= last_cell) {  // cell f-1: Eq. 29, x then y then z (R2)
+          const long long c = idx - sA;
+          cp_async_wait_all();
+          double rho = stage[0][tid], En = stage[4][tid];
+          double m[3] = {stage[1][tid], stage[2][tid], stage[3][tid]};
+#pragma unroll
+          for (int a = 0; a < 2; a++) {
+            const double *q = &stage[5 + 10 * a][tid];
+            rho -= dtd[a] * (q[1 * 128] - q[0 * 128]);
+            m[a] -= dtd[a] * (q[3 * 128] - q[2 * 128]);
+            m[(a + 1) % 3] -= dtd[a] * (q[5 * 128] - q[4 * 128]);
+            m[(a + 2) % 3] -= dtd[a] * (q[7 * 128] - q[6 * 128]);
+            En -= dtd[a] * (q[9 * 128] - q[8 * 128]);
+          }
+          rho -= dtd[2] * (fl.m - fprev.m);
+          m[2] -= dtd[2] * (fl.mn - fprev.mn);
+          m[0] -= dtd[2] * (fl.mt1 - fprev.mt1);
+          m[1] -= dtd[2] * (fl.mt2 - fprev.mt2);
+          En -= dtd[2] * (fl.e - fprev.e);
+          U.f[F_RHO][c] = rho; U.f[F_MX][c] = m[0]; U.f[F_MY][c] = m[1]; U.f[F_MZ][c] = m[2];
+          U.f[F_E][c] = En;
+        }
+        fprev = fl;
+      }
+    }
+    if (UPDATE && upd_col && f >= f0 && f <= last_cell) {  // fetch what cell f's update will need
+      cp_async8(&stage[0][tid], U.f[F_RHO] + idx); cp_async8(&stage[1][tid], U.f[F_MX] + idx);
+      cp_async8(&stage[2][tid], U.f[F_MY] + idx); cp_async8(&stage[3][tid], U.f[F_MZ] + idx);
+      cp_async8(&stage[4][tid], U.f[F_E] + idx);
+#pragma unroll
+      for (int a = 0; a < 2; a++)
+#pragma unroll
+        for (int q = 0; q < 5; q++) {
+          cp_async8(&stage[5 + 10 * a + 2 * q][tid], F.f[a][q] + idx);
+          cp_async8(&stage[5 + 10 * a + 2 * q + 1][tid], F.f[a][q] + idx + g.s[a]);
+        }
+      cp_async_commit();
     }
     WL = hi;
   }
