@@ -208,6 +208,20 @@ def make_problem_name(workload):
     return None, names.get(workload.lower(), workload + " turbulence cube")
 
 
+def job_value(ms_local, cells_per_rank, steps, world, device="cuda"):
+    """Whole-job throughput of N independent replicas ("replicas only"): every
+    rank advances its own grid; the job's time is the MAX over ranks of the device-timed region and
+    the job's work the SUM of the cell updates.  Returns (cell updates/s, ms)."""
+    ms = float(ms_local)
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        t = torch.tensor([ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return world * cells_per_rank * steps / (ms * 1e-3), ms
+
+
 def load_measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -260,11 +274,7 @@ def run_b200(args):
         ms = e0.elapsed_time(e1)
         launches = g.launch_count() - l0
         clocks = sampler.stop() if rank == 0 else None
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        value = world * nc * args.steps / (ms * 1e-3)
+        value, ms = job_value(ms, nc, args.steps, world)
 
         # ---- per-kernel live timing (CUDA events on the library stream) ----------------
         prof = {}
@@ -305,11 +315,7 @@ def run_b200(args):
         torch.cuda.synchronize()
         wall = time.perf_counter() - t0
         ms_e2e = max(e0.elapsed_time(e1), wall * 1e3)
-        if world > 1:
-            t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e2e = float(t.item())
-        e2e_val = world * nc * args.e2e_steps / (ms_e2e * 1e-3)
+        e2e_val, ms_e2e = job_value(ms_e2e, nc, args.e2e_steps, world)
 
     fp64_tf, copy_gbs = (None, None)
     if rank == 0:

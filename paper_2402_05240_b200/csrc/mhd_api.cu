@@ -28,6 +28,12 @@ struct Context {
   cudaStream_t stream = 0;
   long long launches = 0;
   bool rate_valid = false;  // sc->rate_bits holds the CFL rate of the current state
+  // CUDA graph of two consecutive {dt; step} passes (after two steps the B ping-pong pointers are
+  // back where they were, so the captured arguments stay valid); used by mhd_advance on small grids
+  cudaGraphExec_t graph[2] = {nullptr, nullptr};  // one per orientation of the B ping-pong
+  double graph_cfl[2] = {0.0, 0.0};
+  long long graph_launches = 0;
+  int parity = 0;  // flips with every step (which set of face arrays holds B^n)
   // per-launch event timing (mhd_step_profile)
   int prof_n = -1;  // -1 = off, else number of launches recorded so far
   cudaEvent_t prof_ev[kMaxProf + 1];
@@ -201,8 +207,45 @@ int step_kernels() {
     k_update<false><<<gridu, 256, 0, C.stream>>>(C.U, out, C.F, C.E, C.Er, g, ab, C.sc, 1.0);
     LAUNCH_CHECK("k_update(B)+cfl");
     for (int a = 0; a < 3; a++) { C.Bnext.f[a] = C.U.f[F_BX + a]; C.U.f[F_BX + a] = out.f[F_BX + a]; }
+    C.parity ^= 1;
     C.rate_valid = true;
   }
+  return MHD_OK;
+}
+
+void drop_graph() {
+  for (int p = 0; p < 2; p++) {
+    if (C.graph[p]) cudaGraphExecDestroy(C.graph[p]);
+    C.graph[p] = nullptr;
+  }
+}
+
+int step_kernels();
+
+// Capture {k_finish_dt; step} x 2 on the library stream.  Launch-latency matters only for grids that
+// fit in L2 (32^3, 256x16x16: ~12 launches of a few microseconds each per step).
+int build_graph(double cfl) {
+  const int p = C.parity;
+  if (C.graph[p]) cudaGraphExecDestroy(C.graph[p]);
+  C.graph[p] = nullptr;
+  cudaGraph_t gr = nullptr;
+  long long l0 = C.launches;
+  CU(cudaStreamBeginCapture(C.stream, cudaStreamCaptureModeRelaxed));
+  int rc = MHD_OK;
+  for (int s = 0; s < 2 && !rc; s++) {
+    k_finish_dt<<<1, 1, 0, C.stream>>>(C.sc, cfl);
+    C.launches++;
+    rc = step_kernels();
+  }
+  cudaError_t e = cudaStreamEndCapture(C.stream, &gr);
+  C.graph_launches = C.launches - l0;
+  C.launches = l0;
+  if (rc) { if (gr) cudaGraphDestroy(gr); return rc; }
+  if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+  e = cudaGraphInstantiate(&C.graph[p], gr, 0);
+  cudaGraphDestroy(gr);
+  if (e != cudaSuccess) { C.graph[p] = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+  C.graph_cfl[p] = cfl;
   return MHD_OK;
 }
 
@@ -316,10 +359,12 @@ int mhd_set_boundary(int axis, int kind) {
   if (axis < 0 || axis > 2 || (kind != MHD_BC_PERIODIC && kind != MHD_BC_OUTFLOW))
     return fail(MHD_ERR_ARG, "mhd_set_boundary: bad argument");
   C.g.bc[axis] = kind;
+  drop_graph();
   return MHD_OK;
 }
 
 int mhd_set_stream(void *cuda_stream) {
+  if (C.stream != (cudaStream_t)cuda_stream) drop_graph();
   C.stream = (cudaStream_t)cuda_stream;
   return MHD_OK;
 }
@@ -374,7 +419,22 @@ int mhd_advance(int n_steps, double cfl, double *t_accum) {
     CU(cudaStreamSynchronize(C.stream));
     t0 = h.t_accum;
   }
-  for (int s = 0; s < n_steps; s++) {
+  int s = 0;
+  const long long ncell = (long long)C.g.n[0] * C.g.n[1] * C.g.n[2];
+  if (C.stream != 0 && n_steps >= 4 && ncell <= (1LL << 21) && C.prof_n < 0) {  // launch-bound sizes only
+    int rc = ensure_rate();
+    if (rc) return rc;
+    const int p = C.parity;
+    if (!C.graph[p] || C.graph_cfl[p] != cfl) {
+      rc = build_graph(cfl);
+      if (rc) return rc;
+    }
+    for (; s + 2 <= n_steps; s += 2) {
+      CU(cudaGraphLaunch(C.graph[p], C.stream));
+      C.launches += C.graph_launches;
+    }
+  }
+  for (; s < n_steps; s++) {
     int rc = ensure_rate();
     if (rc) return rc;
     k_finish_dt<<<1, 1, 0, C.stream>>>(C.sc, cfl);
@@ -493,6 +553,7 @@ int mhd_synchronize(void) {
 int mhd_finalize(void) {
   if (C.inited) {
     cudaStreamSynchronize(C.stream);
+    drop_graph();
     if (C.owns_memory && C.base) cudaFree(C.base);
   }
   cudaStream_t s = C.stream;

@@ -206,6 +206,12 @@ __device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const
 #ifndef MHD_MINB_FM
 #define MHD_MINB_FM 4
 #endif
+#ifndef MHD_MINB_FM_PPM
+#define MHD_MINB_FM_PPM 3
+#endif
+#ifndef MHD_MINB_FX_PPM
+#define MHD_MINB_FX_PPM 4
+#endif
 __global__ void __launch_bounds__(128, MHD_MINB_PRED) k_predictor_flux(State8 U, Flux21 F, Edge3 Er, Geo g, Box box) {
   const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -385,7 +391,7 @@ __device__ __forceinline__ void reconstruct(double gamma, const W7 *win, double 
 __device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
 template <int R>
-__global__ void __launch_bounds__(128, MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb, int nwx) {
+__global__ void __launch_bounds__(128, R == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb, int nwx) {
   const int lane = threadIdx.x & 31;
   const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int ly = fb.hi[1] - fb.lo[1] + 1, lz = fb.hi[2] - fb.lo[2] + 1;
@@ -440,7 +446,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // do, for the CT kernel), and the full update that follows only has the face field left to do.
 // A chunk then also solves face f1+1 (its last cell needs it; 1/J more Riemann solves).
 template <int A, int R, bool UPDATE>
-__global__ void __launch_bounds__(128, MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
+__global__ void __launch_bounds__(128, R == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
                                                                   State8 U, const Scalars *sc) {
   static_assert(!UPDATE || A == 2, "the fused hydro update rides on the z sweep");
   constexpr int O = (A == 1) ? 2 : 1;  // the other transverse axis

@@ -264,6 +264,33 @@ def test_advance_matches_stepwise_and_device_io(mhd):
     g.close()
 
 
+@pytest.mark.parametrize("recon,bc", [(1, (0, 0, 0)), (2, (1, 0, 0))])
+def test_advance_graph_path_is_bitwise_the_stepwise_path(mhd, recon, bc):
+    """On a non-default stream and a small grid mhd_advance replays a CUDA graph of two steps; an odd
+    step count, a second call (other orientation of the B ping-pong) and a boundary change in between
+    must all give exactly what the kernel-by-kernel path gives."""
+    import torch
+    p = inputs.random_smooth(n=(33, 20, 17), seed=12, recon=recon)
+    ref = mhd.Mhd(*p.n, p.gamma, p.recon, bc)           # default stream: no graph
+    ref.set_state(p.state)
+    for _ in range(7 + 6):
+        ref.step(ref.compute_dt(0.4))
+    want = ref.get_state()
+    ref.close()
+    stream = torch.cuda.Stream()
+    g = mhd.Mhd(*p.n, p.gamma, p.recon, bc, stream=stream)
+    g.set_state(p.state)
+    n0 = g.launch_count()
+    g.advance(7, 0.4)                                    # 3 graph launches + 1 plain step
+    n7 = g.launch_count() - n0
+    g.advance(6, 0.4)                                    # graph for the other parity
+    got = g.get_state()
+    for f in FIELDS:
+        assert np.array_equal(got[f], want[f]), f
+    assert n7 >= 7 * 12                                   # launch_count() counts replayed kernels too
+    g.close()
+
+
 def test_internal_cudamalloc_and_stream(mhd):
     import torch
     p = inputs.random_smooth(n=(20, 12, 10), seed=9, recon=2)
