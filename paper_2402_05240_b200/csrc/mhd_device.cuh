@@ -285,11 +285,10 @@ __device__ __forceinline__ double vl_slope(double dl, double dr) {  // Eq. 26 (G
 }
 
 __device__ __forceinline__ double plm_limit(double aL, double aR, double aC, double aVL) {  // Eq. 27
-  if (aL * aR > 0.0) {
-    double m = fmin(fmin(2.0 * fabs(aL), 2.0 * fabs(aR)), fmin(fabs(aC), fabs(aVL)));
-    return (aC > 0.0) ? m : ((aC < 0.0) ? -m : 0.0);
-  }
-  return 0.0;
+  // min(2|aL|, 2|aR|, |aC|, |aVL|) with the sign of aC; where aL aR > 0, aC = (aL + aR)/2 has their
+  // sign and is non-zero, so the sign transfer is a bit operation
+  double m = fmin(2.0 * fmin(fabs(aL), fabs(aR)), fmin(fabs(aC), fabs(aVL)));
+  return (aL * aR > 0.0) ? copysign(m, aC) : 0.0;
 }
 
 __device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, const W7 &Wp,

@@ -38,10 +38,15 @@ __device__ __forceinline__ double rsqrt_(double x) {
   return y;
 }
 
-// sqrt(x) for normal x > 0, and exactly 0 for x == 0 (x < 0 is the caller's bug).  Branch-free:
-// for x == 0 the seed is +inf and the NaN that follows is discarded by the final select.
+// sqrt(x) for normal x > 0, and exactly 0 for x == 0 (x < 0 is the caller's bug).  One Newton step
+// on the seed (error 2^-44) and then the coupled correction s += (x - s^2) y / 2, which squares the
+// error again: the reciprocal root itself never needs full precision here.  Branch-free: for x == 0
+// the seed is +inf and the NaN that follows is discarded by the final select.
 __device__ __forceinline__ double sqrt_(double x) {
-  double y = rsqrt_(x);
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = __fma_rn(-(0.5 * x) * y, y, 0.5);
+  y = __fma_rn(y, e, y);
   double s = x * y;
   double r = __fma_rn(-s, s, x);  // residual x - s^2
   s = __fma_rn(r, 0.5 * y, s);
