@@ -194,6 +194,9 @@ __device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const
 #ifndef MHD_MINB_UPD
 #define MHD_MINB_UPD 2
 #endif
+#ifndef MHD_MINB_UPDB
+#define MHD_MINB_UPDB 6
+#endif
 #ifndef MHD_MINB_CT
 #define MHD_MINB_CT 3
 #endif
@@ -278,7 +281,7 @@ __device__ __forceinline__ double face_update(const State8 &U, const Edge3 &E, c
 }
 
 template <bool HALF>
-__global__ void __launch_bounds__(256, MHD_MINB_UPD) k_update(State8 Ubase, State8 Uout, Flux21 F, Edge3 E, Edge3 Er,
+__global__ void __launch_bounds__(256, HALF ? MHD_MINB_UPD : MHD_MINB_UPDB) k_update(State8 Ubase, State8 Uout, Flux21 F, Edge3 E, Edge3 Er,
                                                 Geo g, Box box, Scalars *sc, double scale) {
   const int lx = box.hi[0] - box.lo[0] + 2, ly = box.hi[1] - box.lo[1] + 2;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
