@@ -21,7 +21,10 @@
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
  * No -ffast-math.
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): T1..T14 of SURVEY.md 8(c).
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): T1..T14 of SURVEY.md 8(c); for the
+ * primitive-variable variants PLMP / PPMP: the scalar
+ * limiter of Eq. 26-28 typed out per component, agreement with PLMC on a single entropy wave,
+ * the scalar PPM per variable, T1, T8 (2nd-order linear-wave convergence) and T10.
  * Parity unpinned (choice among valid variants, no author code or printed
  * numbers to compare against): HLLD wave-speed estimate and degeneracy
  * tolerance (G15), eigenvector normalisation in degenerate states (G16), the
@@ -319,6 +322,32 @@ void oracle_plmc(double gamma, const double Wm[7], const double W0[7],
 }
 
 /* ------------------------------------------------------------------ */
+/* PLMP ("To limit in the primitive variables instead ...  */
+/* skip steps 3 and 5"): Eq. 23-26, then the limiter of Eq. 27 applied   */
+/* to the primitive differences themselves, then Eq. 28.                 */
+/* ------------------------------------------------------------------ */
+void oracle_plmp(const double Wm[7], const double W0[7], const double Wp[7],
+                 double Wlo[7], double Whi[7])
+{
+    int c;
+    for (c = 0; c < 7; c++) {
+        double dL = W0[c] - Wm[c];                      /* Eq. 23 */
+        double dR = Wp[c] - W0[c];                      /* Eq. 24 */
+        double dC = (Wp[c] - Wm[c]) / 2.0;              /* Eq. 25 */
+        double dVL = (dL * dR > 0.0) ? 2.0 * dL * dR / (dL + dR) : 0.0; /* Eq. 26 */
+        double dm = 0.0;
+        if (dL * dR > 0.0) {                            /* Eq. 27 on delta W */
+            double m = fmin(fmin(2.0 * fabs(dL), 2.0 * fabs(dR)),
+                            fmin(fabs(dC), fabs(dVL)));
+            double sg = (dC > 0.0) ? 1.0 : ((dC < 0.0) ? -1.0 : 0.0);
+            dm = sg * m;
+        }
+        Whi[c] = W0[c] + dm / 2.0;                      /* Eq. 28 */
+        Wlo[c] = W0[c] - dm / 2.0;
+    }
+}
+
+/* ------------------------------------------------------------------ */
 /* O10: PPMC (reading G17 of Felker & Stone 2018, cited PAPER.md:231).  */
 /* One characteristic variable: q[0..4] = q_{i-2..i+2}.                 */
 /* ------------------------------------------------------------------ */
@@ -394,6 +423,18 @@ void oracle_ppmc(double gamma, const double *Ws, double bx0,
     matvec7(R, qhi, Whi);
 }
 
+/* PPMP (PAPER.md:263 applied to the PPM of O10): the same limited parabola,
+ * variable by variable on the primitives, no characteristic projection. */
+void oracle_ppmp(const double *Ws, double Wlo[7], double Whi[7])
+{
+    int s, c;
+    for (c = 0; c < 7; c++) {
+        double qq[5];
+        for (s = 0; s < 5; s++) qq[s] = Ws[s * 7 + c];
+        oracle_ppm_scalar(qq, &Wlo[c], &Whi[c]);
+    }
+}
+
 /* ------------------------------------------------------------------ */
 /* O6: CT edge field, Eq. 15-18 (readings G5-G7).     */
 /* Edge along c at (ia-1/2, ib-1/2), (a,b,c) cyclic.                    */
@@ -431,7 +472,8 @@ typedef struct {
     int n[3], ng, N[3];
     long s[3], ntot;
     double gamma, d[3];
-    int recon;     /* 0 PCM, 1 PLMC, 2 PPMC */
+    int recon;     /* 0 PCM, 1 PLMC, 2 PPMC, 3 PLMP, 4 PPMP */
+    int radius;    /* stencil radius of the reconstruction: 0, 1, 2, 1, 2 */
     int bc[3];     /* 0 periodic, 1 outflow */
     double *U[NF];    /* state at t^n */
     double *Uh[NF];   /* state at t^{n+1/2} */
@@ -456,11 +498,12 @@ int oracle_finalize(void)
 int oracle_init(int nx, int ny, int nz, double gamma, int recon)
 {
     int a, c, f;
-    if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || recon < 0 || recon > 2) return -1;
+    if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || recon < 0 || recon > 4) return -1;
     oracle_finalize();
     G.n[0] = nx; G.n[1] = ny; G.n[2] = nz;
     G.recon = recon;
-    G.ng = 3 + recon; /* stencil radius: PCM 0, PLMC 1, PPMC 2 */
+    G.radius = (recon == 0) ? 0 : ((recon == 1 || recon == 3) ? 1 : 2);
+    G.ng = 3 + G.radius; /* stencil radius: PCM 0, PLMC/PLMP 1, PPMC/PPMP 2 */
     G.gamma = gamma;
     for (a = 0; a < 3; a++) {
         G.N[a] = G.n[a] + 2 * G.ng;
@@ -636,7 +679,7 @@ int oracle_compute_dt(double cfl, double *dt)
 
 /* Steps 2-3 / 6-7: interface states and HLLD flux on every a-face whose
  * stencil is available.  Face (index i along a) lies between cells i-1, i.
- * recon: 0 PCM (Eq. 14), 1 PLMC (O8), 2 PPMC (O10). */
+ * recon: 0 PCM (Eq. 14), 1 PLMC (O8), 2 PPMC (O10), 3 PLMP, 4 PPMP. */
 static void reconstruct_cell(const Grid *g, double *const U[NF], long idx, int a,
                              int recon, double Wlo[7], double Whi[7])
 {
@@ -645,12 +688,14 @@ static void reconstruct_cell(const Grid *g, double *const U[NF], long idx, int a
     if (recon == 0) {
         cell_W(g, U, idx, a, W[2], &bn[2]);
         for (c = 0; c < 7; c++) { Wlo[c] = W[2][c]; Whi[c] = W[2][c]; }
-    } else if (recon == 1) {
+    } else if (recon == 1 || recon == 3) {
         for (s = 1; s <= 3; s++) cell_W(g, U, idx + (s - 2) * g->s[a], a, W[s], &bn[s]);
-        oracle_plmc(g->gamma, W[1], W[2], W[3], bn[2], Wlo, Whi);
+        if (recon == 1) oracle_plmc(g->gamma, W[1], W[2], W[3], bn[2], Wlo, Whi);
+        else oracle_plmp(W[1], W[2], W[3], Wlo, Whi);
     } else {
         for (s = 0; s <= 4; s++) cell_W(g, U, idx + (s - 2) * g->s[a], a, W[s], &bn[s]);
-        oracle_ppmc(g->gamma, (const double *)W, bn[2], Wlo, Whi);
+        if (recon == 2) oracle_ppmc(g->gamma, (const double *)W, bn[2], Wlo, Whi);
+        else oracle_ppmp((const double *)W, Wlo, Whi);
     }
 }
 
@@ -757,7 +802,7 @@ static void update(Grid *g, double *const Ubase[NF], double *Uout[NF], double dt
 int oracle_step(double dt)
 {
     Grid *g = &G;
-    int a, c, x, r = g->recon, ng = g->ng;
+    int a, c, x, r = g->radius, ng = g->ng;
     int lo[3], hi[3], elo[3][3], ehi[3][3], clo[3], chi[3], flo[3][3], fhi[3][3];
     if (!g->inited) return -2;
     if (!(dt > 0.0)) return -1;
@@ -792,7 +837,7 @@ int oracle_step(double dt)
     for (a = 0; a < 3; a++) {
         for (x = 0; x < 3; x++) { lo[x] = -ng + 1; hi[x] = g->n[x] + ng - 2; }
         lo[a] = -ng + 2 + r; hi[a] = g->n[a] + ng - 2 - r;
-        sweep_fluxes(g, g->Uh, a, r, lo, hi);
+        sweep_fluxes(g, g->Uh, a, g->recon, lo, hi);
     }
     /* Step 8 (G12) */
     for (c = 0; c < 3; c++)

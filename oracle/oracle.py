@@ -39,6 +39,8 @@ def lib():
         L.oracle_plmc.argtypes = [_d, _dp, _dp, _dp, _d, _dp, _dp]
         L.oracle_plmc.restype = None
         L.oracle_ppmc.argtypes = [_d, _dp, _d, _dp, _dp]
+        L.oracle_plmp.argtypes = [_dp, _dp, _dp, _dp, _dp]
+        L.oracle_ppmp.argtypes = [_dp, _dp, _dp]
         L.oracle_ppmc.restype = None
         L.oracle_ppm_scalar.argtypes = [_dp, _dp, _dp]
         L.oracle_ppm_scalar.restype = None
@@ -93,6 +95,20 @@ def ppmc(gamma, Ws, bx0):
     Ws = _vec(Ws, 35)
     lo = np.empty(7); hi = np.empty(7)
     lib().oracle_ppmc(gamma, _p(Ws), float(bx0), _p(lo), _p(hi))
+    return lo, hi
+
+
+def plmp(Wm, W0, Wp):
+    Wm = _vec(Wm, 7); W0 = _vec(W0, 7); Wp = _vec(Wp, 7)
+    lo = np.empty(7); hi = np.empty(7)
+    lib().oracle_plmp(_p(Wm), _p(W0), _p(Wp), _p(lo), _p(hi))
+    return lo, hi
+
+
+def ppmp(Ws):
+    Ws = _vec(Ws, 35)
+    lo = np.empty(7); hi = np.empty(7)
+    lib().oracle_ppmp(_p(Ws), _p(lo), _p(hi))
     return lo, hi
 
 

@@ -373,3 +373,56 @@ def test_T7_ct_edge_upwind_selection():
     # Er00 is cell (ia, ib): T1 when Ma0<0, T3 when Mb0<0
     assert call(Er00=1.0, Ma0=-1.0, Mb0=-1.0) == pytest.approx(-0.5)
     assert call(Er00=1.0, Ma0=1.0, Mb0=1.0) == 0.0
+
+
+# ----------------------------------------------------------------------------- PLMP / PPMP
+def test_plmp_is_eq27_on_primitive_differences():
+    """limiting in the primitive variables skips the projections; every component
+    is then the scalar limiter of Eq. 26-28, typed out here, independent of the other six."""
+    rng = np.random.default_rng(12)
+    for _ in range(200):
+        W0 = rand_state(rng)
+        dl, dr = 0.3 * rng.normal(size=7), 0.3 * rng.normal(size=7)
+        lo, hi = orc.plmp(W0 - dl, W0, W0 + dr)
+        for c in range(7):
+            if dl[c] * dr[c] > 0:
+                dc, dvl = 0.5 * (dl[c] + dr[c]), 2 * dl[c] * dr[c] / (dl[c] + dr[c])
+                m = np.sign(dc) * min(2 * abs(dl[c]), 2 * abs(dr[c]), abs(dc), abs(dvl))
+            else:
+                m = 0.0
+            assert hi[c] == pytest.approx(W0[c] + 0.5 * m, abs=1e-15)
+            assert lo[c] == pytest.approx(W0[c] - 0.5 * m, abs=1e-15)
+    # uniform slope is kept, an extremum is flattened, faces stay between the neighbours
+    W0 = rand_state(rng); d = 1e-2 * rng.normal(size=7)
+    lo, hi = orc.plmp(W0 - d, W0, W0 + d)
+    np.testing.assert_allclose(hi, W0 + 0.5 * d, atol=1e-15); np.testing.assert_allclose(lo, W0 - 0.5 * d, atol=1e-15)
+    lo, hi = orc.plmp(W0 + d, W0, W0 + d)
+    np.testing.assert_array_equal(lo, W0); np.testing.assert_array_equal(hi, W0)
+
+
+def test_plmp_equals_plmc_for_a_single_entropy_wave():
+    """Where only rho varies the characteristic and primitive limiters coincide (one wave family,
+    L and R act as the identity on it)."""
+    W0 = np.array([1.0, 0.3, 0.1, -0.2, 0.7, 0.5, 0.4])
+    for dl, dr in ((0.1, 0.3), (0.3, 0.1), (-0.1, -0.4), (0.1, -0.1)):
+        Wm, Wp = W0.copy(), W0.copy()
+        Wm[0] -= dl; Wp[0] += dr
+        a = orc.plmp(Wm, W0, Wp); b = orc.plmc(G, Wm, W0, Wp, 0.6)
+        np.testing.assert_allclose(a[0], b[0], atol=1e-15); np.testing.assert_allclose(a[1], b[1], atol=1e-15)
+
+
+def test_ppmp_is_the_scalar_ppm_per_primitive_variable():
+    rng = np.random.default_rng(13)
+    for _ in range(100):
+        Ws = np.array([rand_state(rng) for _ in range(5)])
+        lo, hi = orc.ppmp(Ws)
+        for c in range(7):
+            l, h = orc.ppm_scalar(Ws[:, c])
+            assert lo[c] == l and hi[c] == h
+    # cubic cell averages without limiter activity: exact 4th-order face values (T11)
+    coef = [0.3, 0.05, 0.01, 0.002]
+    q = np.array([cell_avg(coef, i) for i in range(-2, 3)])
+    Ws = np.tile(q[:, None], (1, 7)) + 2.0
+    lo, hi = orc.ppmp(Ws)
+    P = np.polynomial.Polynomial(coef)
+    assert hi[0] == pytest.approx(P(0.5) + 2.0, abs=1e-14) and lo[3] == pytest.approx(P(-0.5) + 2.0, abs=1e-14)
