@@ -43,6 +43,8 @@ extern "C" {
 #define MHD_RECON_PCM 0  /* Eq. 14, PAPER.md:139-147 (debug: first order everywhere) */
 #define MHD_RECON_PLMC 1 /* Eq. 23-28 */
 #define MHD_RECON_PPMC 2 /* PAPER.md:231, 431; reading O10 */
+#define MHD_RECON_PLMP 3 /* PLM limited in the primitive variables */
+#define MHD_RECON_PPMP 4 /* PPM limited in the primitive variables */
 
 #define MHD_BC_PERIODIC 0
 #define MHD_BC_OUTFLOW 1 /* zero-gradient copy of the nearest active cell/face (O12) */
@@ -145,9 +147,9 @@ int mhd_measure_peaks(double *fp64_tflops, double *copy_gbs, double seconds);
 int mhd_unit_hlld(int n, double gamma, const double *WL, const double *WR, const double *bx,
                   double *F);
 
-/* n independent reconstructions of one cell: recon = MHD_RECON_PLMC (Eq. 23-28, PAPER.md:229-263;
- * stencil of 3 states) or MHD_RECON_PPMC (reading O10; stencil of 5 states).  Ws holds
- * n * (2*recon+1) * 7 values (stencil cell fastest after the component), bn0 the n cell-centred
+/* n independent reconstructions of one cell: recon = MHD_RECON_PLMC / MHD_RECON_PLMP (Eq. 23-28,
+ * PAPER.md:229-263; stencil of 3 states) or MHD_RECON_PPMC / MHD_RECON_PPMP (reading O10; stencil of 5
+ * states).  Ws holds n * (stencil) * 7 values (stencil cell fastest after the component), bn0 the n cell-centred
  * normal fields of the middle cell.  Wlo = W_{R,i-1/2}, Whi = W_{L,i+1/2}, n*7 values each. */
 int mhd_unit_reconstruct(int n, double gamma, int recon, const double *Ws, const double *bn0,
                          double *Wlo, double *Whi);

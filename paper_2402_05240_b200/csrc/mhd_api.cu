@@ -73,9 +73,9 @@ int cuda_fail(cudaError_t e, const char *where) {
 inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 bool make_geo(Geo &g, int nx, int ny, int nz, double gamma, int recon) {
-  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || recon < 0 || recon > 2) return false;
+  if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || recon < 0 || recon > 4) return false;
   g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
-  g.ng = 3 + recon;  // stencil radius: PCM 0, PLMC 1, PPMC 2
+  g.ng = 3 + recon_radius(recon);  // stencil radius: PCM 0, PLMC/PLMP 1, PPMC/PPMP 2
   g.ox = round_up(g.ng, 4);
   g.N[0] = round_up(g.ox + nx + g.ng, 8);
   g.N[1] = ny + 2 * g.ng;
@@ -122,7 +122,7 @@ Box make_box(int l0, int h0, int l1, int h1, int l2, int h2) {
   return b;
 }
 
-template <int R>
+template <int RC>
 int launch_corrector_fluxes() {
   const Geo &g = C.g;
   const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
@@ -131,7 +131,7 @@ int launch_corrector_fluxes() {
     Box fb = make_box(0, n0, -1, n1, -1, n2);
     int nwx = (n0 + 1 + 30) / 31;  // warps per pencil: 31 faces each, faces 0..n0
     long long nw = (long long)nwx * (n1 + 2) * (n2 + 2);
-    k_flux_x<R><<<grid1(nw, 4), 128, 0, C.stream>>>(C.Uh, C.F, g, fb, nwx);
+    k_flux_x<RC><<<grid1(nw, 4), 128, 0, C.stream>>>(C.Uh, C.F, g, fb, nwx);
     LAUNCH_CHECK("k_flux_x");
   }
   {
@@ -142,7 +142,7 @@ int launch_corrector_fluxes() {
 #endif
     long long nt = (long long)(n0 + 2) * (n2 + 2);
     dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
-    k_flux_march<1, R, false><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
+    k_flux_march<1, RC, false><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<1>");
   }
   {
@@ -150,7 +150,7 @@ int launch_corrector_fluxes() {
     int J = (n2 + 1 >= 64) ? 32 : ((n2 + 1 >= 16) ? 8 : 4);
     long long nt = (long long)(n0 + 2) * (n1 + 2);
     dim3 grid(grid1(nt, 128).x, (n2 + 1 + J - 1) / J);
-    k_flux_march<2, R, true><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
+    k_flux_march<2, RC, true><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<2>+update");
   }
   return MHD_OK;
@@ -159,7 +159,7 @@ int launch_corrector_fluxes() {
 // One VL+CT step with the dt held in C.sc->dt.
 int step_kernels() {
   const Geo &g = C.g;
-  const int r = g.recon;
+  const int r = recon_radius(g.recon);
   int rc = fill_ghosts(C.U);  // one boundary update per step
   if (rc) return rc;
   // Steps 2-3: PCM + HLLD on cells [-2-r, n+r+1]
@@ -186,9 +186,13 @@ int step_kernels() {
     LAUNCH_CHECK("k_update(half)");
   }
   // Steps 6-7: reconstruction + HLLD from U^{n+1/2}
-  if (r == 0) rc = launch_corrector_fluxes<0>();
-  else if (r == 1) rc = launch_corrector_fluxes<1>();
-  else rc = launch_corrector_fluxes<2>();
+  switch (g.recon) {
+    case 0: rc = launch_corrector_fluxes<0>(); break;
+    case 1: rc = launch_corrector_fluxes<1>(); break;
+    case 2: rc = launch_corrector_fluxes<2>(); break;
+    case 3: rc = launch_corrector_fluxes<3>(); break;
+    default: rc = launch_corrector_fluxes<4>(); break;
+  }
   if (rc) return rc;
   // Step 8 (G12): CT with the corrector fluxes and the half-step reference state, indices [0, n]
   // Step 9: full update of cells [0, n-1] and faces 0..n

@@ -321,6 +321,18 @@ __device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, c
 #undef MHD_O
 }
 
+// PLMP (limiting in the primitive variables = Eq. 23-28 without the projections)
+__device__ __forceinline__ void plmp(const W7 &Wm, const W7 &W0, const W7 &Wp, W7 &Wlo, W7 &Whi) {
+#define MHD_P1(f)                                                                        \
+  {                                                                                      \
+    double dl = W0.f - Wm.f, dr = Wp.f - W0.f;                                           \
+    double dm = plm_limit(dl, dr, 0.5 * (dl + dr), vl_slope(dl, dr));                    \
+    Whi.f = W0.f + 0.5 * dm; Wlo.f = W0.f - 0.5 * dm;                                    \
+  }
+  MHD_P1(rho) MHD_P1(u) MHD_P1(v) MHD_P1(w) MHD_P1(P) MHD_P1(by) MHD_P1(bz)
+#undef MHD_P1
+}
+
 // ---------------------------------------------------------------------------------------
 // PPMC (reading O10 / G17 of Felker & Stone 2018, cited PAPER.md:231, 431).
 // ---------------------------------------------------------------------------------------
@@ -391,6 +403,18 @@ __device__ __forceinline__ void ppmc(double gamma, const W7 &Wm2, const W7 &Wm1,
   ppm_scalar(q0.c6, q1.c6, q2.c6, q3.c6, q4.c6, lo.c6, hi.c6);
   Wlo = eig_right(e, lo);
   Whi = eig_right(e, hi);
+}
+
+// PPMP (PAPER.md:263 applied to the PPM of O10): the limited parabola per primitive variable
+__device__ __forceinline__ void ppmp(const W7 &Wm2, const W7 &Wm1, const W7 &W0, const W7 &Wp1, const W7 &Wp2,
+                                     W7 &Wlo, W7 &Whi) {
+  ppm_scalar(Wm2.rho, Wm1.rho, W0.rho, Wp1.rho, Wp2.rho, Wlo.rho, Whi.rho);
+  ppm_scalar(Wm2.u, Wm1.u, W0.u, Wp1.u, Wp2.u, Wlo.u, Whi.u);
+  ppm_scalar(Wm2.v, Wm1.v, W0.v, Wp1.v, Wp2.v, Wlo.v, Whi.v);
+  ppm_scalar(Wm2.w, Wm1.w, W0.w, Wp1.w, Wp2.w, Wlo.w, Whi.w);
+  ppm_scalar(Wm2.P, Wm1.P, W0.P, Wp1.P, Wp2.P, Wlo.P, Whi.P);
+  ppm_scalar(Wm2.by, Wm1.by, W0.by, Wp1.by, Wp2.by, Wlo.by, Whi.by);
+  ppm_scalar(Wm2.bz, Wm1.bz, W0.bz, Wp1.bz, Wp2.bz, Wlo.bz, Whi.bz);
 }
 
 // ---------------------------------------------------------------------------------------

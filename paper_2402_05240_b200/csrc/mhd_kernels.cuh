@@ -379,11 +379,16 @@ __global__ void __launch_bounds__(256) k_divb(State8 U, Geo g, unsigned long lon
 // PAPER.md:307): each cell is reconstructed once, its upper-face state W_{L,i+1/2} is handed
 // to the thread / iteration that owns face i+1/2.
 // ---------------------------------------------------------------------------------------
-template <int R>
+// recon code RC (include/mhd.h MHD_RECON_*) -> stencil radius: PCM 0, PLMC/PLMP 1, PPMC/PPMP 2
+__host__ __device__ constexpr int recon_radius(int rc) { return rc == 0 ? 0 : ((rc == 1 || rc == 3) ? 1 : 2); }
+
+template <int RC>
 __device__ __forceinline__ void reconstruct(double gamma, const W7 *win, double bn0, W7 &lo, W7 &hi) {
-  if (R == 0) { lo = win[0]; hi = win[0]; }                                   // Eq. 14
-  else if (R == 1) plmc(gamma, win[0], win[1], win[2], bn0, lo, hi);          // Eq. 23-28
-  else ppmc(gamma, win[0], win[1], win[2], win[3], win[4], bn0, lo, hi);      // O10
+  if (RC == 0) { lo = win[0]; hi = win[0]; }                                   // Eq. 14
+  else if (RC == 1) plmc(gamma, win[0], win[1], win[2], bn0, lo, hi);          // Eq. 23-28
+  else if (RC == 2) ppmc(gamma, win[0], win[1], win[2], win[3], win[4], bn0, lo, hi);  // O10
+  else if (RC == 3) plmp(win[0], win[1], win[2], lo, hi);
+  else ppmp(win[0], win[1], win[2], win[3], win[4], lo, hi);
 }
 
 // x sweep: one WARP per 31 consecutive faces of an x pencil.  Lane l reconstructs cell c0 + l
@@ -393,8 +398,9 @@ __device__ __forceinline__ void reconstruct(double gamma, const W7 *win, double 
 // overlap by one cell (1/31 of the reconstructions are done twice).
 __device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
-template <int R>
-__global__ void __launch_bounds__(128, R == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb, int nwx) {
+template <int RC>
+__global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb, int nwx) {
+  constexpr int R = recon_radius(RC);
   const int lane = threadIdx.x & 31;
   const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int ly = fb.hi[1] - fb.lo[1] + 1, lz = fb.hi[2] - fb.lo[2] + 1;
@@ -414,7 +420,7 @@ __global__ void __launch_bounds__(128, R == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) k
       Prim p = load_prim_half(Uh, g, idx + (s - R));
       win[s] = to_W<0>(p, bnc[s]);
     }
-    reconstruct<R>(g.gamma, win, bnc[R], lo, hi);
+    reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
   } else {
     hi.rho = hi.u = hi.v = hi.w = hi.P = hi.by = hi.bz = 0.0;
     lo = hi;
@@ -448,10 +454,11 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // The four momentum / energy z fluxes then never go to memory (the mass and magnetic fluxes still
 // do, for the CT kernel), and the full update that follows only has the face field left to do.
 // A chunk then also solves face f1+1 (its last cell needs it; 1/J more Riemann solves).
-template <int A, int R, bool UPDATE>
-__global__ void __launch_bounds__(128, R == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
+template <int A, int RC, bool UPDATE>
+__global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
                                                                   State8 U, const Scalars *sc) {
   static_assert(!UPDATE || A == 2, "the fused hydro update rides on the z sweep");
+  constexpr int R = recon_radius(RC);
   constexpr int O = (A == 1) ? 2 : 1;  // the other transverse axis
   const int lx = fb.hi[0] - fb.lo[0] + 1, lo_ = fb.hi[O] - fb.lo[O] + 1;
   long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -497,7 +504,7 @@ __global__ void __launch_bounds__(128, R == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) k
       Prim p = load_prim_half(Uh, g, idx + (long long)R * sA);
       win[2 * R] = to_W<A>(p, bnc[2 * R]);
     }
-    reconstruct<R>(g.gamma, win, bnc[R], lo, hi);
+    reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
     if (f >= f0) {
       F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX + A] + idx));
       if (!UPDATE) {

@@ -32,15 +32,18 @@ __global__ void k_unit_hlld(int n, double gamma, const double *WL, const double 
   o[0] = f.m; o[1] = f.mn; o[2] = f.mt1; o[3] = f.mt2; o[4] = f.e; o[5] = f.by; o[6] = f.bz;
 }
 
-template <int R>
+template <int RC>
 __global__ void k_unit_recon(int n, double gamma, const double *Ws, const double *bn0, double *Wlo,
                              double *Whi) {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
   W7 lo, hi;
+  constexpr int R = (RC == 1 || RC == 3) ? 1 : 2;
   const double *s = Ws + (size_t)t * 7 * (2 * R + 1);
-  if (R == 1) plmc(gamma, load_W(s), load_W(s + 7), load_W(s + 14), bn0[t], lo, hi);
-  else ppmc(gamma, load_W(s), load_W(s + 7), load_W(s + 14), load_W(s + 21), load_W(s + 28), bn0[t], lo, hi);
+  if (RC == 1) plmc(gamma, load_W(s), load_W(s + 7), load_W(s + 14), bn0[t], lo, hi);
+  else if (RC == 2) ppmc(gamma, load_W(s), load_W(s + 7), load_W(s + 14), load_W(s + 21), load_W(s + 28), bn0[t], lo, hi);
+  else if (RC == 3) plmp(load_W(s), load_W(s + 7), load_W(s + 14), lo, hi);
+  else ppmp(load_W(s), load_W(s + 7), load_W(s + 14), load_W(s + 21), load_W(s + 28), lo, hi);
   store_W(Wlo + 7 * t, lo);
   store_W(Whi + 7 * t, hi);
 }
@@ -82,14 +85,17 @@ extern "C" int mhd_unit_hlld(int n, double gamma, const double *WL, const double
 
 extern "C" int mhd_unit_reconstruct(int n, double gamma, int recon, const double *Ws, const double *bn0,
                                     double *Wlo, double *Whi) {
-  if (n < 0 || !Ws || !bn0 || !Wlo || !Whi || !(gamma > 1.0) || (recon != 1 && recon != 2)) return MHD_ERR_ARG;
+  if (n < 0 || !Ws || !bn0 || !Wlo || !Whi || !(gamma > 1.0) || recon < 1 || recon > 4) return MHD_ERR_ARG;
   if (n == 0) return MHD_OK;
-  const size_t ns = 7 * (size_t)(2 * recon + 1) * n;
+  const int radius = (recon == 1 || recon == 3) ? 1 : 2;
+  const size_t ns = 7 * (size_t)(2 * radius + 1) * n;
   DevBuf a, b, c, d;
   if (!a.alloc(ns) || !b.alloc(n) || !c.alloc(7 * (size_t)n) || !d.alloc(7 * (size_t)n)) return MHD_ERR_NOMEM;
   if (!a.up(Ws, ns) || !b.up(bn0, n)) return MHD_ERR_CUDA;
   if (recon == 1) k_unit_recon<1><<<(n + 127) / 128, 128>>>(n, gamma, a.p, b.p, c.p, d.p);
-  else k_unit_recon<2><<<(n + 127) / 128, 128>>>(n, gamma, a.p, b.p, c.p, d.p);
+  else if (recon == 2) k_unit_recon<2><<<(n + 127) / 128, 128>>>(n, gamma, a.p, b.p, c.p, d.p);
+  else if (recon == 3) k_unit_recon<3><<<(n + 127) / 128, 128>>>(n, gamma, a.p, b.p, c.p, d.p);
+  else k_unit_recon<4><<<(n + 127) / 128, 128>>>(n, gamma, a.p, b.p, c.p, d.p);
   if (cudaGetLastError() != cudaSuccess || !c.down(Wlo, 7 * (size_t)n) || !d.down(Whi, 7 * (size_t)n)) return MHD_ERR_CUDA;
   return MHD_OK;
 }

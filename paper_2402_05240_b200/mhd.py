@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 # MHD_LIBRARY overrides the in-tree build (e.g. to compare two builds of the same ABI)
 LIB_PATH = os.environ.get("MHD_LIBRARY") or os.path.join(_HERE, "libmhd.so")
 
-RECON_PCM, RECON_PLMC, RECON_PPMC = 0, 1, 2
+RECON_PCM, RECON_PLMC, RECON_PPMC, RECON_PLMP, RECON_PPMP = 0, 1, 2, 3, 4
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = ctypes.POINTER(ctypes.c_double)
@@ -106,7 +106,8 @@ def unit_hlld(gamma, WL, WR, bx):
 
 def unit_reconstruct(gamma, recon, Ws, bn0):
     """n reconstructions on the device: Ws (n, 2*recon+1, 7), bn0 (n,) -> (Wlo, Whi), (n,7) each."""
-    Ws = np.ascontiguousarray(Ws, dtype=np.float64).reshape(-1, 2 * recon + 1, 7)
+    radius = 1 if recon in (RECON_PLMC, RECON_PLMP) else 2
+    Ws = np.ascontiguousarray(Ws, dtype=np.float64).reshape(-1, 2 * radius + 1, 7)
     bn0 = np.ascontiguousarray(bn0, dtype=np.float64).reshape(-1)
     n = Ws.shape[0]
     if bn0.shape[0] != n:

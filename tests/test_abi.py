@@ -43,7 +43,7 @@ def test_argument_errors_without_a_device(libpath):
     L.mhd_workspace_bytes.restype = ctypes.c_size_t
     L.mhd_last_error.restype = ctypes.c_char_p
     assert L.mhd_workspace_bytes(0, 4, 4, 1) == 0
-    assert L.mhd_workspace_bytes(4, 4, 4, 3) == 0
+    assert L.mhd_workspace_bytes(4, 4, 4, 5) == 0
     # 40 arrays of pitch 40 (4 + 32 + 4) * 40 * 40 doubles, PLMC ng = 4
     nbytes = L.mhd_workspace_bytes(32, 32, 32, 1)
     assert nbytes >= 40 * 40 * 40 * 40 * 8

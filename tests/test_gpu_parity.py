@@ -58,7 +58,7 @@ def test_roundtrip_set_get(mhd):
     g.close()
 
 
-@pytest.mark.parametrize("recon", [0, 1, 2])
+@pytest.mark.parametrize("recon", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("n", [(37, 21, 19), (130, 9, 34), (16, 70, 5)])
 def test_one_step_random_smooth(mhd, recon, n):
     """Ragged sizes spanning several x-pencil blocks (127 faces) and march chunks."""
@@ -76,7 +76,7 @@ def test_one_step_random_smooth(mhd, recon, n):
     o.close(); g.close()
 
 
-@pytest.mark.parametrize("recon", [1, 2])
+@pytest.mark.parametrize("recon", [1, 2, 3, 4])
 def test_uniform_state_bit_for_bit(mhd, recon):
     p = inputs.uniform(n=(8, 6, 5), recon=recon)
     g = mhd.Mhd(*p.n, p.gamma, p.recon)
@@ -91,7 +91,7 @@ def test_uniform_state_bit_for_bit(mhd, recon):
 
 
 @pytest.mark.parametrize("n", [(1, 1, 1), (2, 1, 3), (5, 3, 2), (4, 4, 4)])
-@pytest.mark.parametrize("recon", [1, 2])
+@pytest.mark.parametrize("recon", [1, 2, 3, 4])
 def test_tiny_grids(mhd, n, recon):
     """Grids thinner than the ghost depth: periodic images wrap more than once."""
     p = inputs.random_smooth(n=(8, 8, 8), seed=5, recon=recon)
@@ -221,6 +221,36 @@ def test_c4_blast_small(mhd):
     rd = rel_diff(out, ref)
     assert max(rd.values()) <= 1e-9, "blast 20 steps free-running: %s" % rd
     o.close(); g.close()
+
+
+@pytest.mark.parametrize("recon", [3, 4])
+def test_primitive_limiting_brio_wu_and_blast_steps(mhd, recon):
+    """PLMP / PPMP on the discontinuous problems: 12 steps of Brio-Wu (outflow x) and
+    8 of the 24^3 blast, every step a one-step parity case from the oracle's own state."""
+    for p, nsteps in ((inputs.riemann("brio_wu", 64, 4, axis=0, recon=recon), 12), (inputs.blast(24, recon=recon), 8)):
+        o, g = make_pair(mhd, p)
+        state = p.state
+        for s in range(nsteps):
+            g.set_state(state)
+            dt = o.compute_dt(p.cfl)
+            o.step(dt); g.step(dt)
+            state = o.get_state()
+            out = g.get_state()
+            what = "%s recon %d step %d" % (p.name, recon, s + 1)
+            if p.name == "blast" and recon == 4:
+                # Reading R7 flushes differences below tau = 1e-12 max|q| in the PPM extremum test; the
+                # flush is itself a switch of size tau.  Ahead of the blast wave, where the perturbation
+                # of the uniform background is itself ~1e-12, oracle and kernels can take different
+                # sides of it in a few cells (seen: 1.2e-12 in one step).  Counted, not waved through:
+                # at most 48 cells per field (the 24 symmetry images of two sites; seen: 24) may exceed 1e-12, none 5e-12.
+                for f in FIELDS:
+                    sc = max(np.abs(state[f]).max(), np.abs(state["rho"]).max() if f in ("mx", "my", "mz") else 0.0)
+                    d = np.abs(out[f] - state[f]) / sc
+                    assert d.max() <= 5e-12 and int((d > TOL_STEP).sum()) <= 48, (what, f, d.max(), int((d > TOL_STEP).sum()))
+            else:
+                assert_close(out, state, TOL_STEP, what)
+            assert divb_normalised(out, p.n) <= TOL_DIVB
+        o.close(); g.close()
 
 
 def test_c3_turbulence_small_multi_step(mhd):
