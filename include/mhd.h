@@ -70,6 +70,11 @@ int mhd_init_workspace(int nx, int ny, int nz, double gamma, int recon, void *wo
  * mhd_set_state* or mhd_step). */
 int mhd_set_boundary(int axis, int kind);
 
+/* Domain lengths L_x, L_y, L_z > 0 (default 1 x 1 x 1): Delta_a = L_a / n_a.  The paper's non-cubic
+ * test boxes keep cubic cells this way (3 x 1.5 x 1.5 at 2N x N x N; 1 x 1 x 2 at
+ * N x N x 2N; 1 x 1.5 x 1 at 200 x 300 x 200). */
+int mhd_set_domain(double lx, double ly, double lz);
+
 /* cudaStream_t (as void*) on which all later work is launched; NULL = default stream. */
 int mhd_set_stream(void *cuda_stream);
 

@@ -525,6 +525,18 @@ int oracle_init(int nx, int ny, int nz, double gamma, int recon)
     return 0;
 }
 
+/* Domain lengths (default 1 x 1 x 1): Delta_a = L_a / n_a.  The paper's non-cubic test boxes
+ * (3 x 1.5 x 1.5; 1 x 1 x 2; 1 x 1.5 x 1) keep cubic cells. */
+int oracle_set_domain(double lx, double ly, double lz)
+{
+    double L[3] = {lx, ly, lz};
+    int a;
+    if (!G.inited) return -2;
+    for (a = 0; a < 3; a++) if (!(L[a] > 0.0)) return -1;
+    for (a = 0; a < 3; a++) G.d[a] = L[a] / G.n[a];
+    return 0;
+}
+
 int oracle_set_boundary(int axis, int kind)
 {
     if (!G.inited) return -2;

@@ -26,6 +26,7 @@ def lib():
         L = ctypes.CDLL(path)
         L.oracle_init.argtypes = [ctypes.c_int] * 3 + [_d, ctypes.c_int]
         L.oracle_set_boundary.argtypes = [ctypes.c_int, ctypes.c_int]
+        L.oracle_set_domain.argtypes = [_d, _d, _d]
         L.oracle_set_state.argtypes = [_dp] * 8
         L.oracle_get_state.argtypes = [_dp] * 8
         L.oracle_get_half_state.argtypes = [_dp] * 8
@@ -148,11 +149,14 @@ def field_shapes(nx, ny, nz):
 class Oracle:
     """One global grid inside liboracle.so (same call sequence as the product ABI)."""
 
-    def __init__(self, nx, ny, nz, gamma, recon, bc=(0, 0, 0)):
+    def __init__(self, nx, ny, nz, gamma, recon, bc=(0, 0, 0), domain=(1.0, 1.0, 1.0)):
         self.n = (nx, ny, nz)
         rc = lib().oracle_init(nx, ny, nz, float(gamma), int(recon))
         if rc:
             raise RuntimeError("oracle_init failed: %d" % rc)
+        if tuple(domain) != (1.0, 1.0, 1.0):
+            if lib().oracle_set_domain(*[float(x) for x in domain]):
+                raise RuntimeError("oracle_set_domain failed")
         for a, kind in enumerate(bc):
             lib().oracle_set_boundary(a, int(kind))
 

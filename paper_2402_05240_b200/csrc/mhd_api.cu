@@ -82,7 +82,7 @@ bool make_geo(Geo &g, int nx, int ny, int nz, double gamma, int recon) {
   g.N[2] = nz + 2 * g.ng;
   g.s[0] = 1; g.s[1] = g.N[0]; g.s[2] = (long long)g.N[0] * g.N[1];
   g.ntot = g.s[2] * g.N[2];
-  for (int a = 0; a < 3; a++) { g.d[a] = 1.0 / g.n[a]; g.bc[a] = MHD_BC_PERIODIC; }
+  for (int a = 0; a < 3; a++) { g.d[a] = 1.0 / g.n[a]; g.id[a] = (double)g.n[a]; g.bc[a] = MHD_BC_PERIODIC; }
   g.gamma = gamma;
   g.gm1inv = 1.0 / (gamma - 1.0);
   g.recon = recon;
@@ -364,6 +364,17 @@ int mhd_set_boundary(int axis, int kind) {
     return fail(MHD_ERR_ARG, "mhd_set_boundary: bad argument");
   C.g.bc[axis] = kind;
   drop_graph();
+  return MHD_OK;
+}
+
+int mhd_set_domain(double lx, double ly, double lz) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  const double L[3] = {lx, ly, lz};
+  for (int a = 0; a < 3; a++)
+    if (!(L[a] > 0.0)) return fail(MHD_ERR_ARG, "mhd_set_domain: lengths must be positive");
+  for (int a = 0; a < 3; a++) { C.g.d[a] = L[a] / C.g.n[a]; C.g.id[a] = C.g.n[a] / L[a]; }
+  drop_graph();
+  C.rate_valid = false;
   return MHD_OK;
 }
 

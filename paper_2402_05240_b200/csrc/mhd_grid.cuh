@@ -32,7 +32,8 @@ struct Geo {
   int N[3];        // allocated extents (N[0] = pitch)
   long long s[3];  // strides
   long long ntot;  // pitch * N[1] * N[2]
-  double d[3];     // Delta_a = 1/n_a
+  double d[3];     // Delta_a = L_a / n_a (unit box by default)
+  double id[3];    // 1 / Delta_a (= n_a exactly on the unit box)
   double gamma;
   double gm1inv;   // 1 / (gamma - 1)
   int bc[3];

@@ -108,7 +108,7 @@ __device__ __forceinline__ double cell_rate(const Geo &g, const Prim &p, int &ba
 #pragma unroll
   for (int a = 0; a < 3; a++) {
     double cf = sqrt_(fast_speed_sq(g.gamma, p.ir, p.P, p.B[a], p.B[(a + 1) % 3], p.B[(a + 2) % 3]));
-    r = fmax(r, (fabs(p.v[a]) + cf) * (double)g.n[a]);  // 1/Delta_a = n_a exactly (unit box)
+    r = fmax(r, (fabs(p.v[a]) + cf) * g.id[a]);
   }
   bad |= !isfinite(r) || !(r > 0.0);
   return r;
@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(256, HALF ? MHD_MINB_UPD : MHD_MINB_UPDB) k_up
   const double dts = scale * sc->dt;
   double dtd[3];
 #pragma unroll
-  for (int a = 0; a < 3; a++) dtd[a] = dts * (double)g.n[a];  // 1/Delta_a = n_a exactly
+  for (int a = 0; a < 3; a++) dtd[a] = dts * g.id[a];
   double Bl[3];
   Bl[0] = (iny && inz) ? face_update<0>(Ubase, E, g, idx, dtd) : 0.0;
   Bl[1] = (inz && inx) ? face_update<1>(Ubase, E, g, idx, dtd) : 0.0;
@@ -474,7 +474,7 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
   if (UPDATE) {
     const double dt = sc->dt;
 #pragma unroll
-    for (int a = 0; a < 3; a++) dtd[a] = dt * (double)g.n[a];
+    for (int a = 0; a < 3; a++) dtd[a] = dt * g.id[a];
   }
   W7 win[2 * R + 1];
   double bnc[2 * R + 1];

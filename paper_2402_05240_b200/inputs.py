@@ -16,6 +16,10 @@ Recipes (DESIGN.md section "Inputs"):
                   motivation, not a paper test
   blast        -- BASELINE.json configs[3]; variant of PAPER.md:455-459
   random_smooth-- small seeded smooth field for parity tests (div B = 0 by construction)
+  cpaw         -- circularly polarised Alfven wave, PAPER.md:358-370
+  field_loop   -- advecting field loop, PAPER.md:378-391 (Eq. 36)
+  orszag_tang  -- PAPER.md:467-475
+  blast_paper  -- MHD blast in the paper's own box, PAPER.md:455-459
 """
 from dataclasses import dataclass, field
 
@@ -36,6 +40,7 @@ class Problem:
     t_end: float = None
     n_steps: int = None
     meta: dict = field(default_factory=dict)
+    domain: tuple = (1.0, 1.0, 1.0)   # box lengths; Delta_a = L_a / n_a
 
 
 def field_shapes(nx, ny, nz):
@@ -364,3 +369,133 @@ def uniform(n=(8, 8, 8), gamma=5.0 / 3.0, rho=1.3, P=0.7, v=(0.3, -0.2, 0.5), B=
     st = from_primitives(rho * c, v[0] * c, v[1] * c, v[2] * c, P * c, np.full(sh["bx"], B[0]),
                          np.full(sh["by"], B[1]), np.full(sh["bz"], B[2]), gamma)
     return Problem(name="uniform", n=tuple(n), gamma=gamma, state=st, recon=recon, n_steps=1)
+
+
+# ------------------------------------------------------------------------------
+# The rest of the paper's test suite.  B always from a vector potential
+# sampled on cell edges and differenced onto faces, so that div B = 0 to round-off
+# (PAPER.md:370, 382, 475).
+# ------------------------------------------------------------------------------
+def _edge_coords(n, L, origin):
+    """Cell-centre and lower-face coordinates along each axis."""
+    c = [origin[a] + (np.arange(n[a]) + 0.5) * L[a] / n[a] for a in range(3)]
+    f = [origin[a] + np.arange(n[a] + 1) * L[a] / n[a] for a in range(3)]
+    return c, f
+
+
+def _curl_to_faces(Ax, Ay, Az, n, L):
+    """Ax on x-edges [k-1/2, j-1/2, i] shape (nz+1, ny+1, nx); Ay (nz+1, ny, nx+1); Az (nz, ny+1, nx+1).
+    Returns face fields bx (nz, ny, nx+1), by (nz, ny+1, nx), bz (nz+1, ny, nx)."""
+    dx, dy, dz = (L[a] / n[a] for a in range(3))
+    bx = (Az[:, 1:, :] - Az[:, :-1, :]) / dy - (Ay[1:, :, :] - Ay[:-1, :, :]) / dz
+    by = (Ax[1:, :, :] - Ax[:-1, :, :]) / dz - (Az[:, :, 1:] - Az[:, :, :-1]) / dx
+    bz = (Ay[:, :, 1:] - Ay[:, :, :-1]) / dx - (Ax[:, 1:, :] - Ax[:, :-1, :]) / dy
+    return bx, by, bz
+
+
+def cpaw(N=16, recon=1, standing=False, amplitude=0.1):
+    """Circularly polarised Alfven wave: periodic 3 x 1.5 x 1.5 box, 2N x N x N
+    cells, rho = 1, P = 0.1, B_1 = 1, transverse v and B of amplitude 0.1 rotating with phase
+    2 pi x_1, x_1 along e_1 = (cos a cos b, cos a sin b, sin a); one period = 1 (Alfven speed 1).
+    sin a = 2/3; sin b is read as 2/sqrt(5) (G25: the printed 1/sqrt(5) is not periodic in
+    this box), so e_1 = (1/3, 2/3, 2/3)."""
+    gamma = 5.0 / 3.0
+    n = (2 * N, N, N)
+    L = (3.0, 1.5, 1.5)
+    sa, sb = 2.0 / 3.0, 2.0 / np.sqrt(5.0)
+    ca, cb = np.sqrt(1 - sa * sa), np.sqrt(1 - sb * sb)
+    e1 = np.array([ca * cb, ca * sb, sa])
+    e2 = np.array([-sb, cb, 0.0])
+    e3 = np.array([-sa * cb, -sa * sb, ca])
+    c, f = _edge_coords(n, L, (0.0, 0.0, 0.0))
+
+    def x1(X, Y, Z):
+        return e1[0] * X + e1[1] * Y + e1[2] * Z
+
+    def grid(zs, ys, xs):
+        return np.meshgrid(zs, ys, xs, indexing="ij")
+
+    A = amplitude
+    k2 = 2.0 * np.pi
+
+    def potential(Z, Y, X):  # wave part of A in the wave frame: (0, A sin/(2 pi), A cos/(2 pi))
+        ph = k2 * x1(X, Y, Z)
+        a2, a3 = A * np.sin(ph) / k2, A * np.cos(ph) / k2
+        return [a2 * e2[i] + a3 * e3[i] for i in range(3)]
+
+    Ax = potential(*grid(f[2], f[1], c[0]))[0]
+    Ay = potential(*grid(f[2], c[1], f[0]))[1]
+    Az = potential(*grid(c[2], f[1], f[0]))[2]
+    bx, by, bz = _curl_to_faces(Ax, Ay, Az, n, L)
+    bx += e1[0]; by += e1[1]; bz += e1[2]     # uniform B_1 = 1 along e_1
+    Zc, Yc, Xc = grid(c[2], c[1], c[0])
+    ph = k2 * x1(Xc, Yc, Zc)
+    v1 = -1.0 if standing else 0.0
+    v2, v3 = A * np.sin(ph), A * np.cos(ph)
+    v = [v1 * e1[i] + v2 * e2[i] + v3 * e3[i] for i in range(3)]
+    rho = np.ones_like(ph)
+    st = from_primitives(rho, v[0], v[1], v[2], 0.1 * rho, bx, by, bz, gamma)
+    return Problem(name="cpaw", n=n, gamma=gamma, state=st, recon=recon, cfl=0.4, t_end=1.0, domain=L,
+                   meta={"standing": standing})
+
+
+def field_loop(N=32, recon=2, amplitude=1e-3, radius=0.3):
+    """Advecting field loop (Eq. 36): periodic 1 x 1 x 2 box centred at zero,
+    N x N x 2N cells, rho = 1, P = 1, v = (1, 1, 2); A_x = 0, A_y = A_z = A (R - r) inside r < R = 0.3
+    (r from the box centre, each component sampled on its own edges), A = 1e-3; two periods, t = 2."""
+    gamma = 5.0 / 3.0
+    n = (N, N, 2 * N)
+    L = (1.0, 1.0, 2.0)
+    c, f = _edge_coords(n, L, (-0.5, -0.5, -1.0))
+
+    def pot(zs, ys, xs):
+        Z, Y, X = np.meshgrid(zs, ys, xs, indexing="ij")
+        r = np.sqrt(X * X + Y * Y + Z * Z)
+        return np.where(r < radius, amplitude * (radius - r), 0.0)
+
+    Ax = np.zeros((n[2] + 1, n[1] + 1, n[0]))
+    Ay = pot(f[2], c[1], f[0])
+    Az = pot(c[2], f[1], f[0])
+    bx, by, bz = _curl_to_faces(Ax, Ay, Az, n, L)
+    one = np.ones((n[2], n[1], n[0]))
+    st = from_primitives(one, 1.0 * one, 1.0 * one, 2.0 * one, one, bx, by, bz, gamma)
+    return Problem(name="field_loop", n=n, gamma=gamma, state=st, recon=recon, cfl=0.4, t_end=2.0, domain=L)
+
+
+def orszag_tang(N=192, nz=None, recon=2):
+    """Orszag-Tang vortex: periodic unit box, rho = 25/(36 pi), P = 5/(12 pi),
+    v = (sin 2 pi y, -sin 2 pi x, 0) as printed, A_z = (B0 / 4 pi)(cos 4 pi x + 2 cos 2 pi y),
+    B0 = 1/sqrt(4 pi); gamma = 5/3 (not stated in the paper; the standard choice); t = 0.5."""
+    gamma = 5.0 / 3.0
+    nz = N if nz is None else nz
+    n = (N, N, nz)
+    L = (1.0, 1.0, 1.0)
+    c, f = _edge_coords(n, L, (0.0, 0.0, 0.0))
+    B0 = 1.0 / np.sqrt(4.0 * np.pi)
+    Zc, Yf, Xf = np.meshgrid(c[2], f[1], f[0], indexing="ij")
+    Az = B0 / (4.0 * np.pi) * (np.cos(4 * np.pi * Xf) + 2.0 * np.cos(2 * np.pi * Yf))
+    Ax = np.zeros((n[2] + 1, n[1] + 1, n[0]))
+    Ay = np.zeros((n[2] + 1, n[1], n[0] + 1))
+    bx, by, bz = _curl_to_faces(Ax, Ay, Az, n, L)
+    Z, Y, X = np.meshgrid(c[2], c[1], c[0], indexing="ij")
+    rho = 25.0 / (36.0 * np.pi) * np.ones_like(X)
+    st = from_primitives(rho, np.sin(2 * np.pi * Y), -np.sin(2 * np.pi * X), np.zeros_like(X),
+                         5.0 / (12.0 * np.pi) * np.ones_like(X), bx, by, bz, gamma)
+    return Problem(name="orszag_tang", n=n, gamma=gamma, state=st, recon=recon, cfl=0.4, t_end=0.5)
+
+
+def blast_paper(nx=200, recon=2, p_in=10.0, p_out=0.1, radius=0.1):
+    """MHD blast wave as the paper runs it: periodic 1 x 1.5 x 1 box, nx x 1.5 nx x nx
+    cells (200 x 300 x 200), rho = 1, v = 0, B = (1, 1, 0)/sqrt(2) (beta = 0.2), P = 10 inside the
+    central sphere of radius 0.1 and 0.1 outside; t = 0.2."""
+    gamma = 5.0 / 3.0
+    n = (nx, (3 * nx) // 2, nx)
+    L = (1.0, 1.5, 1.0)
+    c, f = _edge_coords(n, L, (-0.5, -0.75, -0.5))
+    Z, Y, X = np.meshgrid(c[2], c[1], c[0], indexing="ij")
+    P = np.where(X * X + Y * Y + Z * Z < radius * radius, p_in, p_out)
+    b = 1.0 / np.sqrt(2.0)
+    one = np.ones_like(X)
+    st = from_primitives(one, 0 * one, 0 * one, 0 * one, P, b * np.ones((n[2], n[1], n[0] + 1)),
+                         b * np.ones((n[2], n[1] + 1, n[0])), np.zeros((n[2] + 1, n[1], n[0])), gamma)
+    return Problem(name="blast_paper", n=n, gamma=gamma, state=st, recon=recon, cfl=0.4, t_end=0.2, domain=L)

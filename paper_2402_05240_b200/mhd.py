@@ -39,6 +39,7 @@ def _load():
     L.mhd_init_workspace.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double, ctypes.c_int, _vp, ctypes.c_size_t]
     L.mhd_set_boundary.argtypes = [ctypes.c_int, ctypes.c_int]
     L.mhd_set_stream.argtypes = [_vp]
+    L.mhd_set_domain.argtypes = [ctypes.c_double] * 3
     L.mhd_set_state.argtypes = [_dp] * 8
     L.mhd_set_state_device.argtypes = [_vp] * 8
     L.mhd_compute_dt.argtypes = [ctypes.c_double, _dp]
@@ -60,7 +61,7 @@ def _load():
     L.mhd_unit_math.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp]
     L.mhd_launch_count.restype = ctypes.c_longlong
     L.mhd_last_error.restype = ctypes.c_char_p
-    for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_stream", "mhd_set_state",
+    for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_domain", "mhd_set_stream", "mhd_set_state",
                  "mhd_set_state_device", "mhd_compute_dt", "mhd_step", "mhd_advance", "mhd_get_state",
                  "mhd_get_state_device", "mhd_get_half_state", "mhd_max_divb", "mhd_synchronize",
                  "mhd_finalize", "mhd_get_flux", "mhd_unit_hlld", "mhd_unit_reconstruct", "mhd_unit_ct_edge", "mhd_unit_math"):
@@ -137,7 +138,7 @@ class Mhd:
     """The single global context of libmhd.so, same call sequence as the C ABI."""
 
     def __init__(self, nx, ny, nz, gamma, recon=RECON_PLMC, bc=(0, 0, 0), use_torch_workspace=True,
-                 stream=None):
+                 stream=None, domain=(1.0, 1.0, 1.0)):
         import torch
         if not torch.cuda.is_available():
             raise MhdError("no CUDA device: the VL+CT step has no CPU fallback")
@@ -160,6 +161,8 @@ class Mhd:
             _check(_lib.mhd_init(nx, ny, nz, float(gamma), int(recon)))
         for a, kind in enumerate(bc):
             _check(_lib.mhd_set_boundary(a, int(kind)))
+        if tuple(domain) != (1.0, 1.0, 1.0):
+            _check(_lib.mhd_set_domain(*[float(x) for x in domain]))
 
     # ---- host-buffer path -------------------------------------------------------------
     def set_state(self, state):

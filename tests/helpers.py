@@ -28,9 +28,9 @@ def run_steps(sim, p, n_steps):
     return dts
 
 
-def divb_normalised(state, n):
+def divb_normalised(state, n, domain=(1.0, 1.0, 1.0)):
     """max |sum_a dB_a/Delta_a| * min(Delta) / B_rms over active cells (SURVEY.md 8(c) parity metric)."""
-    nx, ny, nz = n
+    nx, ny, nz = (n[a] / domain[a] for a in range(3))   # 1 / Delta_a
     bx, by, bz = state["bx"], state["by"], state["bz"]
     div = ((bx[:, :, 1:] - bx[:, :, :-1]) * nx + (by[:, 1:, :] - by[:, :-1, :]) * ny
            + (bz[1:, :, :] - bz[:-1, :, :]) * nz)

@@ -23,9 +23,9 @@ def mhd():
 
 
 def make_pair(mhd, p, **kw):
-    o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc)
+    o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc, p.domain)
     o.set_state(p.state)
-    g = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc, **kw)
+    g = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc, domain=p.domain, **kw)
     g.set_state(p.state)
     return o, g
 

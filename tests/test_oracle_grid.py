@@ -22,7 +22,7 @@ GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
 
 def make(p):
-    o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc)
+    o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc, p.domain)
     o.set_state(p.state)
     return o
 
