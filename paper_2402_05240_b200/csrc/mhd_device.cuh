@@ -209,9 +209,17 @@ __device__ __forceinline__ void eig_setup(Eig &e, double gamma, const W7 &W, dou
   double cf2 = (s + sqrt_(disc)) * (0.5 * irho);  // Eq. 12
   double ca2 = bx * bx * irho;
   double cs2 = (cf2 > 0.0) ? a2 * ca2 * rcp(cf2) : 0.0;  // slow speed without cancellation (O9)
-  double cf = sqrt_(cf2), cs = sqrt_(cs2);
-  if (bp2 == 0.0) { e.betay = 1.0; e.betaz = 0.0; }
-  else { double ib = rsqrt_(bp2); e.betay = W.by * ib; e.betaz = W.bz * ib; }
+  double cf = sqrt_(cf2), cs = sqrt_any(cs2);  // c_s^2 ~ B_n^2 can be denormal
+  if (bp2 == 0.0 && W.by == 0.0 && W.bz == 0.0) { e.betay = 1.0; e.betaz = 0.0; }
+  else {
+    // the numerical foot ahead of a switch-on shock carries transverse fields down to 1e-180 and
+    // below (Ryu & Jones 4d): rescale before squaring so that the seed instruction never sees a
+    // denormal (it flushes them to zero and the direction would come out as inf * 0)
+    double by = W.by, bz = W.bz;
+    if (fmax(fabs(by), fabs(bz)) < 0x1p-500) { by *= 0x1p600; bz *= 0x1p600; }
+    double ib = rsqrt_(by * by + bz * bz);
+    e.betay = by * ib; e.betaz = bz * ib;
+  }
   double dfs = cf2 - cs2;
   if (dfs == 0.0) { e.alf = 1.0; e.als = 0.0; }
   else {
@@ -377,7 +385,7 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
     double s = sgn3(Df);
     if (s != 0.0 && s == sgn3(Dm1) && s == sgn3(D0) && s == sgn3(Dp1))
       Dlim = s * fmin(fmin(C * fabs(Dm1), C * fabs(D0)), fmin(C * fabs(Dp1), fabs(Df)));
-    if (fabs(Df) > tau) r = Dlim * rcp(Df);
+    if (fabs(Df) > fmax(tau, 1e-290)) r = Dlim * rcp(Df);  // (the floor keeps rcp off denormals)
     if (r <= 1.0 - 1e-12) { qm = qi - r * dm; qp = qi + r * dp; }
   } else {
     if (fabs(dm) >= 2.0 * fabs(dp)) qm = qi - 2.0 * dp;

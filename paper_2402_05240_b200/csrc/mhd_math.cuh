@@ -53,6 +53,16 @@ __device__ __forceinline__ double sqrt_(double x) {
   return (x == 0.0) ? 0.0 : s;
 }
 
+// sqrt(x) for x >= 0 of ANY magnitude, denormals included (the seed instruction flushes them to
+// zero): operands below 2^-900 are scaled by 2^200 first.  For the one call site that can meet such
+// values -- the slow speed where the normal field is ~1e-160 in the numerical foot of a switch-on
+// shock (Ryu & Jones 4d).
+__device__ __forceinline__ double sqrt_any(double x) {
+  const bool tiny = x < 0x1p-900;
+  double s = sqrt_(tiny ? x * 0x1p200 : x);
+  return tiny ? s * 0x1p-100 : s;
+}
+
 // sqrt(x) and 1/sqrt(x) together, x > 0.
 __device__ __forceinline__ void sqrt_rsqrt(double x, double &s, double &is) {
   double y = rsqrt_(x);
