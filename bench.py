@@ -167,7 +167,7 @@ def sample_problem(workload):
     if w == "c4":
         return inputs.blast(64, recon=2), "c4 recipe (blast, PPMC) at 64^3"
     recon = 2 if w.endswith(":ppmc") else 1
-    return inputs.turbulence(96, recon=recon), "c3/c5 recipe (Mach-1 beta-1 turbulence, recon=%d) at 96^3" % recon
+    return inputs.turbulence(128, recon=recon), "c3/c5 recipe (Mach-1 beta-1 turbulence, recon=%d) at 128^3" % recon
 
 
 def run_reference(args):
@@ -373,7 +373,7 @@ def run_b200(args):
                 "paper_context": {"a100_cell_updates_per_s": 2.59e8, "ratio": value / world / 2.59e8}}
         if world == 1 and not args.no_cpu_baseline:
             sp, sname = sample_problem(args.workload)
-            v, el, cores = time_oracle(sp, 6 if sp.n[0] >= 64 else 40)
+            v, el, cores = time_oracle(sp, 20 if sp.n[0] >= 64 else 400)   # ~10-20 s of host work
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": sname + ", %.1f s" % el}
         print(json.dumps(line))
