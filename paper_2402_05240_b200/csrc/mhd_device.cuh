@@ -347,6 +347,10 @@ __device__ __forceinline__ void plmp(const W7 &Wm, const W7 &W0, const W7 &Wp, W
 __device__ __forceinline__ double sgn3(double x) { return (x > 0.0) ? 1.0 : ((x < 0.0) ? -1.0 : 0.0); }
 
 // limited 4th-order value on the face between cells j and j+1; qa..qd = q_{j-1..j+2}
+// "D_f and the cell curvatures share a sign" is tested with products (a fp64 multiply and a compare
+// each, instead of three-way sign extraction), and sgn * min(C|D_a|, C|D_b|, |D_f|) is formed as
+// copysign(min(C min(|D_a|, |D_b|), |D_f|), D_f): multiplication by C = 1.25 is monotone, so the
+// value is bit for bit the oracle's.
 __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, double qd) {
   const double C = 1.25;
   double qf = (7.0 / 12.0) * (qb + qc) - (1.0 / 12.0) * (qa + qd);
@@ -354,10 +358,9 @@ __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, doub
     double Df = 3.0 * (qb - 2.0 * qf + qc);
     double Dj = qa - 2.0 * qb + qc;
     double Dj1 = qb - 2.0 * qc + qd;
-    double s = sgn3(Df);
     double Dlim = 0.0;
-    if (s != 0.0 && s == sgn3(Dj) && s == sgn3(Dj1))
-      Dlim = s * fmin(fmin(C * fabs(Dj), C * fabs(Dj1)), fabs(Df));
+    if (Df * Dj > 0.0 && Df * Dj1 > 0.0)
+      Dlim = copysign(fmin(C * fmin(fabs(Dj), fabs(Dj1)), fabs(Df)), Df);
     qf = 0.5 * (qb + qc) - Dlim * (1.0 / 6.0);
   }
   return qf;
@@ -382,9 +385,8 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
     double D0 = q1 - 2.0 * q2 + q3;
     double Dp1 = q2 - 2.0 * q3 + q4;
     double Dlim = 0.0, r = 0.0;
-    double s = sgn3(Df);
-    if (s != 0.0 && s == sgn3(Dm1) && s == sgn3(D0) && s == sgn3(Dp1))
-      Dlim = s * fmin(fmin(C * fabs(Dm1), C * fabs(D0)), fmin(C * fabs(Dp1), fabs(Df)));
+    if (Df * Dm1 > 0.0 && Df * D0 > 0.0 && Df * Dp1 > 0.0)
+      Dlim = copysign(fmin(C * fmin(fabs(Dm1), fmin(fabs(D0), fabs(Dp1))), fabs(Df)), Df);
     if (fabs(Df) > fmax(tau, 1e-290)) r = Dlim * rcp(Df);  // (the floor keeps rcp off denormals)
     if (r <= 1.0 - 1e-12) { qm = qi - r * dm; qp = qi + r * dp; }
   } else {
