@@ -294,15 +294,19 @@ __global__ void __launch_bounds__(256, HALF ? MHD_MINB_UPD : MHD_MINB_UPDB) k_up
   double dtd[3];
 #pragma unroll
   for (int a = 0; a < 3; a++) dtd[a] = dts * g.id[a];
+  // evaluated unconditionally (every operand lies inside the padded arrays; results of indices
+  // that do not own the face are simply not stored): no branch ahead of the loads, so all of the
+  // kernel's ~60 loads go out in one batch -- this kernel lives on loads in flight
   double Bl[3];
-  Bl[0] = (iny && inz) ? face_update<0>(Ubase, E, g, idx, dtd) : 0.0;
-  Bl[1] = (inz && inx) ? face_update<1>(Ubase, E, g, idx, dtd) : 0.0;
-  Bl[2] = (inx && iny) ? face_update<2>(Ubase, E, g, idx, dtd) : 0.0;
+  Bl[0] = face_update<0>(Ubase, E, g, idx, dtd);
+  Bl[1] = face_update<1>(Ubase, E, g, idx, dtd);
+  Bl[2] = face_update<2>(Ubase, E, g, idx, dtd);
   double rate = 0.0;
   int bad = 0;
-  if (inx && iny && inz) {
-    double rho = Ubase.f[F_RHO][idx], En = Ubase.f[F_E][idx];
-    double m[3] = {Ubase.f[F_MX][idx], Ubase.f[F_MY][idx], Ubase.f[F_MZ][idx]};
+  const bool in_cell = inx && iny && inz;
+  {
+    double rho = __ldg(Ubase.f[F_RHO] + idx), En = __ldg(Ubase.f[F_E] + idx);
+    double m[3] = {__ldg(Ubase.f[F_MX] + idx), __ldg(Ubase.f[F_MY] + idx), __ldg(Ubase.f[F_MZ] + idx)};
     if (HALF) {  // Eq. 19; in the full step the z sweep has already applied Eq. 29 to these five
 #pragma unroll
       for (int a = 0; a < 3; a++) {
@@ -324,12 +328,14 @@ __global__ void __launch_bounds__(256, HALF ? MHD_MINB_UPD : MHD_MINB_UPDB) k_up
 #pragma unroll
     for (int a = 0; a < 3; a++) p.v[a] = m[a] * p.ir;
     p.P = pressure(g.gamma - 1.0, rho, p.v, En, p.B);
-    if (HALF) {
-      Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = p.v[0]; Uout.f[F_MY][idx] = p.v[1];
-      Uout.f[F_MZ][idx] = p.v[2]; Uout.f[F_E][idx] = p.P;
-      store_eref(Er, idx, p);
-    } else {
-      rate = cell_rate(g, p, bad);
+    if (in_cell) {
+      if (HALF) {
+        Uout.f[F_RHO][idx] = rho; Uout.f[F_MX][idx] = p.v[0]; Uout.f[F_MY][idx] = p.v[1];
+        Uout.f[F_MZ][idx] = p.v[2]; Uout.f[F_E][idx] = p.P;
+        store_eref(Er, idx, p);
+      } else {
+        rate = cell_rate(g, p, bad);
+      }
     }
   }
   // the face arrays of Uout are never those of Ubase (the upper-face reads above would race)
