@@ -65,18 +65,22 @@ __device__ __forceinline__ double pressure(double gm1, double rho, const double 
 
 // O1 from the CONSERVED state U^n: v = m / rho, cell-centred B = mean of
 // the two opposing faces (Eq. 13), P from the total energy.
-__device__ __forceinline__ Prim load_prim(const State8 &U, const Geo &g, long long idx) {
+__device__ __forceinline__ Prim make_prim(double gm1, double rho, double mx, double my, double mz, double E,
+                                          double bxl, double bxh, double byl, double byh, double bzl, double bzh) {
   Prim p;
-  double rho = __ldg(U.f[F_RHO] + idx);
   double ir = rcp(rho);
   p.rho = rho; p.ir = ir;
-#pragma unroll
-  for (int a = 0; a < 3; a++) {
-    p.B[a] = 0.5 * (__ldg(U.f[F_BX + a] + idx) + __ldg(U.f[F_BX + a] + idx + g.s[a]));
-    p.v[a] = __ldg(U.f[F_MX + a] + idx) * ir;
-  }
-  p.P = pressure(g.gamma - 1.0, rho, p.v, __ldg(U.f[F_E] + idx), p.B);
+  p.B[0] = 0.5 * (bxl + bxh); p.B[1] = 0.5 * (byl + byh); p.B[2] = 0.5 * (bzl + bzh);
+  p.v[0] = mx * ir; p.v[1] = my * ir; p.v[2] = mz * ir;
+  p.P = pressure(gm1, rho, p.v, E, p.B);
   return p;
+}
+
+__device__ __forceinline__ Prim load_prim(const State8 &U, const Geo &g, long long idx) {
+  return make_prim(g.gamma - 1.0, __ldg(U.f[F_RHO] + idx), __ldg(U.f[F_MX] + idx), __ldg(U.f[F_MY] + idx),
+                   __ldg(U.f[F_MZ] + idx), __ldg(U.f[F_E] + idx), __ldg(U.f[F_BX] + idx),
+                   __ldg(U.f[F_BX] + idx + g.s[0]), __ldg(U.f[F_BY] + idx), __ldg(U.f[F_BY] + idx + g.s[1]),
+                   __ldg(U.f[F_BZ] + idx), __ldg(U.f[F_BZ] + idx + g.s[2]));
 }
 
 // The half-step state is held in PRIMITIVE form (rho, v, P at cell centres in slots F_RHO..F_E,

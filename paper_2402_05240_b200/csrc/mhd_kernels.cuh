@@ -171,6 +171,17 @@ __device__ __forceinline__ void store_eref(const Edge3 &Er, long long idx, const
   Er.f[2][idx] = -(p.v[0] * p.B[1] - p.v[1] * p.B[0]);
 }
 
+// Asynchronous 8-byte global -> shared copies (LDGSTS) into a per-thread column of shared memory:
+// operands that are needed later (the neighbour cells of the predictor, the fused hydro update of
+// the z sweep) are requested early, and their HBM latency hides behind a Riemann solve or a whole
+// reconstruction at no cost in registers.
+__device__ __forceinline__ void cp_async8(double *smem, const double *gmem) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 // ---------------------------------------------------------------------------------------
 // a2: predictor.  One thread per cell of `box`; it forms the PCM states (Eq. 14)
 // of its own cell and of its three lower neighbours and solves HLLD on its three lower faces
@@ -178,10 +189,27 @@ __device__ __forceinline__ void store_eref(const Edge3 &Er, long long idx, const
 // Face a is skipped where the lower neighbour lies outside the box.  The thread also leaves
 // the reference field of its cell (Eq. 18) for the CT kernel.
 // ---------------------------------------------------------------------------------------
+#define MHD_PRED_T 128
+// neighbour cell `slot` (0, 1, 2 = lower x, y, z neighbour) of the calling thread, staged by cp.async
+__device__ __forceinline__ void stage_cell(double (*st)[MHD_PRED_T], int slot, const State8 &U, const Geo &g,
+                                           long long c) {
+  const int t = threadIdx.x, o = 11 * slot;
+  cp_async8(&st[o + 0][t], U.f[F_RHO] + c); cp_async8(&st[o + 1][t], U.f[F_MX] + c);
+  cp_async8(&st[o + 2][t], U.f[F_MY] + c); cp_async8(&st[o + 3][t], U.f[F_MZ] + c);
+  cp_async8(&st[o + 4][t], U.f[F_E] + c);
+#pragma unroll
+  for (int b = 0; b < 3; b++) {
+    cp_async8(&st[o + 5 + 2 * b][t], U.f[F_BX + b] + c);
+    cp_async8(&st[o + 6 + 2 * b][t], U.f[F_BX + b] + c + g.s[b]);
+  }
+}
+
 template <int A>
-__device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const Geo &g,
+__device__ __forceinline__ void pcm_face(double (*st)[MHD_PRED_T], const State8 &U, const Flux21 &F, const Geo &g,
                                          long long idx, const Prim &pc) {
-  Prim pm = load_prim(U, g, idx - g.s[A]);
+  const int t = threadIdx.x, o = 11 * A;
+  Prim pm = make_prim(g.gamma - 1.0, st[o][t], st[o + 1][t], st[o + 2][t], st[o + 3][t], st[o + 4][t], st[o + 5][t],
+                      st[o + 6][t], st[o + 7][t], st[o + 8][t], st[o + 9][t], st[o + 10][t]);
   double bn;
   W7 WL = to_W<A>(pm, bn);
   W7 WR = to_W<A>(pc, bn);
@@ -215,17 +243,25 @@ __device__ __forceinline__ void pcm_face(const State8 &U, const Flux21 &F, const
 #ifndef MHD_MINB_FX_PPM
 #define MHD_MINB_FX_PPM 4
 #endif
-__global__ void __launch_bounds__(128, MHD_MINB_PRED) k_predictor_flux(State8 U, Flux21 F, Edge3 Er, Geo g, Box box) {
+__global__ void __launch_bounds__(MHD_PRED_T, MHD_MINB_PRED) k_predictor_flux(State8 U, Flux21 F, Edge3 Er, Geo g, Box box) {
+  __shared__ double st[33][MHD_PRED_T];
   const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= lx * ly) return;
   int i = box.lo[0] + t % lx, j = box.lo[1] + t / lx, k = box.lo[2] + blockIdx.y;
   long long idx = cell_index(g, i, j, k);
+  // the three lower neighbours are requested first (they lie inside the arrays even for the first
+  // layer of the box, whose faces are not solved); the thread's own cell goes through registers
+  stage_cell(st, 0, U, g, idx - g.s[0]);
+  stage_cell(st, 1, U, g, idx - g.s[1]);
+  stage_cell(st, 2, U, g, idx - g.s[2]);
+  cp_async_commit();
   Prim pc = load_prim(U, g, idx);
   store_eref(Er, idx, pc);
-  if (i > box.lo[0]) pcm_face<0>(U, F, g, idx, pc);
-  if (j > box.lo[1]) pcm_face<1>(U, F, g, idx, pc);
-  if (k > box.lo[2]) pcm_face<2>(U, F, g, idx, pc);
+  cp_async_wait_all();
+  if (i > box.lo[0]) pcm_face<0>(st, U, F, g, idx, pc);
+  if (j > box.lo[1]) pcm_face<1>(st, U, F, g, idx, pc);
+  if (k > box.lo[2]) pcm_face<2>(st, U, F, g, idx, pc);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -439,16 +475,6 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) 
     store_flux<0>(F, idx, f);
   }
 }
-
-// Asynchronous 8-byte global -> shared copies (LDGSTS): the operands of the fused hydro update are
-// fetched one marching iteration ahead into a per-thread column of shared memory, so their HBM
-// latency hides behind a whole reconstruction + Riemann solve at no cost in registers.
-__device__ __forceinline__ void cp_async8(double *smem, const double *gmem) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // y / z sweep: a thread owns one x position (warps run along x, so every load and store is
 // coalesced) and marches along the sweep axis over a chunk of J faces with a rolling window
