@@ -181,6 +181,8 @@ __device__ __forceinline__ void cp_async8(double *smem, const double *gmem) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+// all groups but the most recently committed one are complete
+__device__ __forceinline__ void cp_async_wait_but_last() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------
 // a2: predictor.  One thread per cell of `box`; it forms the PCM states (Eq. 14)
@@ -526,6 +528,26 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
   const int tid = threadIdx.x;
   const int last_cell = min(f1, g.n[A] - 1);
   idx -= sA;
+  // The cell that enters the window in iteration f (cell f + R) is requested one iteration earlier
+  // into this thread's column of `pre` (double-buffered): rho, v, P and the six faces around it.
+  // cp.async groups complete in order and every iteration commits exactly two (the prefetch, then
+  // the update operands -- either may be empty), so "all but the last group" is always the right wait.
+  // Used by the 3-cell (PLM) sweeps; the 5-cell PPM sweeps are register-bound and lose with it.
+  constexpr bool PREF = (R == 1);
+  __shared__ double pre[PREF ? 2 : 1][PREF ? 11 : 1][PREF ? 128 : 1];
+  auto prefetch = [&](int buf, long long c) {
+    cp_async8(&pre[buf][0][tid], Uh.f[F_RHO] + c); cp_async8(&pre[buf][1][tid], Uh.f[F_MX] + c);
+    cp_async8(&pre[buf][2][tid], Uh.f[F_MY] + c); cp_async8(&pre[buf][3][tid], Uh.f[F_MZ] + c);
+    cp_async8(&pre[buf][4][tid], Uh.f[F_E] + c);
+#pragma unroll
+    for (int b = 0; b < 3; b++) {
+      cp_async8(&pre[buf][5 + 2 * b][tid], Uh.f[F_BX + b] + c);
+      cp_async8(&pre[buf][6 + 2 * b][tid], Uh.f[F_BX + b] + c + g.s[b]);
+    }
+  };
+  if (PREF) prefetch((f0 - 1) & 1, idx + (long long)R * sA);
+  cp_async_commit();
+  cp_async_commit();  // (empty: keeps the two-groups-per-iteration count from the start)
   // One reconstruct() call site per kernel: iteration f0-1 only produces W_L of face f0; every
   // cell is then reconstructed by the same instruction sequence, so mirror-image cells give
   // mirror-image states bit for bit.
@@ -533,8 +555,22 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
 #pragma unroll
     for (int s = 0; s < 2 * R; s++) { win[s] = win[s + 1]; bnc[s] = bnc[s + 1]; }
     {
-      Prim p = load_prim_half(Uh, g, idx + (long long)R * sA);
+      Prim p;
+      if (PREF) {
+        cp_async_wait_but_last();  // the prefetch of this iteration's cell (the newer group is the update's)
+        const int b = f & 1;
+        p.rho = pre[b][0][tid]; p.ir = 0.0;
+        p.v[0] = pre[b][1][tid]; p.v[1] = pre[b][2][tid]; p.v[2] = pre[b][3][tid];
+        p.P = pre[b][4][tid];
+        p.B[0] = 0.5 * (pre[b][5][tid] + pre[b][6][tid]);
+        p.B[1] = 0.5 * (pre[b][7][tid] + pre[b][8][tid]);
+        p.B[2] = 0.5 * (pre[b][9][tid] + pre[b][10][tid]);
+        if (f < fend) prefetch(b ^ 1, idx + (long long)(R + 1) * sA);
+      } else {
+        p = load_prim_half(Uh, g, idx + (long long)R * sA);
+      }
       win[2 * R] = to_W<A>(p, bnc[2 * R]);
+      cp_async_commit();
     }
     reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
     if (f >= f0) {
@@ -545,7 +581,7 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
         if (f <= f1) { F.f[A][0][idx] = fl.m; F.f[A][5][idx] = fl.by; F.f[A][6][idx] = fl.bz; }
         if (upd_col && f > f0 && f - 1 <= last_cell) {  // cell f-1: Eq. 29, x then y then z (R2)
           const long long c = idx - sA;
-          cp_async_wait_all();
+          cp_async_wait_but_last();  // its operands (the newer group is the next cell's prefetch)
           double rho = stage[0][tid], En = stage[4][tid];
           double m[3] = {stage[1][tid], stage[2][tid], stage[3][tid]};
 #pragma unroll
@@ -579,8 +615,8 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
           cp_async8(&stage[5 + 10 * a + 2 * q][tid], F.f[a][q] + idx);
           cp_async8(&stage[5 + 10 * a + 2 * q + 1][tid], F.f[a][q] + idx + g.s[a]);
         }
-      cp_async_commit();
     }
+    cp_async_commit();  // always: one update group per iteration, possibly empty
     WL = hi;
   }
 }
