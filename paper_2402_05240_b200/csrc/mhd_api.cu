@@ -125,6 +125,8 @@ Box make_box(int l0, int h0, int l1, int h1, int l2, int h2) {
 template <int RC>
 int launch_corrector_fluxes() {
   const Geo &g = C.g;
+  // the 5-cell sweeps keep their window in dynamic shared memory (opt-in above 48 KB for the z sweep)
+  const size_t wsm = (recon_radius(RC) == 2) ? (size_t)MHD_WSM_BYTES : 0;  // opted in at mhd_init
   const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
   // faces 0..n along the sweep, transverse -1..n (what CT and the final update need)
   {
@@ -142,7 +144,7 @@ int launch_corrector_fluxes() {
 #endif
     long long nt = (long long)(n0 + 2) * (n2 + 2);
     dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
-    k_flux_march<1, RC, false><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
+    k_flux_march<1, RC, false><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<1>");
   }
   {
@@ -150,7 +152,7 @@ int launch_corrector_fluxes() {
     int J = (n2 + 1 >= 64) ? 32 : ((n2 + 1 >= 16) ? 8 : 4);
     long long nt = (long long)(n0 + 2) * (n1 + 2);
     dim3 grid(grid1(nt, 128).x, (n2 + 1 + J - 1) / J);
-    k_flux_march<2, RC, true><<<grid, 128, 0, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
+    k_flux_march<2, RC, true><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<2>+update");
   }
   return MHD_OK;
@@ -267,8 +269,20 @@ int ensure_rate() {
   return MHD_OK;
 }
 
+// the 5-cell sweeps use more than 48 KB of shared memory per block (window + update operands)
+template <int RC>
+int opt_in_shared_memory() {
+  CU(cudaFuncSetAttribute(k_flux_march<1, RC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, MHD_WSM_BYTES));
+  CU(cudaFuncSetAttribute(k_flux_march<2, RC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, MHD_WSM_BYTES));
+  return MHD_OK;
+}
+
 int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_t ws_bytes) {
   mhd_finalize();
+  if (recon == MHD_RECON_PPMC || recon == MHD_RECON_PPMP) {
+    int rc = (recon == MHD_RECON_PPMC) ? opt_in_shared_memory<2>() : opt_in_shared_memory<4>();
+    if (rc) return rc;
+  }
   Geo g;
   if (!make_geo(g, nx, ny, nz, gamma, recon)) return fail(MHD_ERR_ARG, "mhd_init: bad argument");
   size_t need = total_bytes(g);

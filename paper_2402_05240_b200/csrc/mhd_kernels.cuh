@@ -478,6 +478,7 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) 
   }
 }
 
+#define MHD_WSM_BYTES (5 * 8 * 128 * 8)
 // y / z sweep: a thread owns one x position (warps run along x, so every load and store is
 // coalesced) and marches along the sweep axis over a chunk of J faces with a rolling window
 // of 2R+1 primitive states in registers; each cell's primitives are formed once per chunk.
@@ -512,13 +513,30 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
   }
   W7 win[2 * R + 1];
   double bnc[2 * R + 1];
+  // 5-cell (PPM) sweeps: the window lives in this thread's column of shared memory (ring of 5 slots)
+  // between iterations, so that its 40 doubles do not sit in registers across the projections
+  // (dynamic shared memory, MHD_WSM_BYTES per block: with the update operands of the z sweep the
+  // total exceeds the 48 KB static limit)
+  constexpr bool WSM = (R == 2);
+  extern __shared__ double wsm_[];
+  auto wput = [&](int slot, const W7 &W, double bn) {
+    double *q = wsm_ + slot * 8 * 128 + threadIdx.x;
+    q[0] = W.rho; q[128] = W.u; q[256] = W.v; q[384] = W.w; q[512] = W.P; q[640] = W.by; q[768] = W.bz; q[896] = bn;
+  };
+  auto wget = [&](int slot, W7 &W, double &bn) {
+    const double *q = wsm_ + slot * 8 * 128 + threadIdx.x;
+    W.rho = q[0]; W.u = q[128]; W.v = q[256]; W.w = q[384]; W.P = q[512]; W.by = q[640]; W.bz = q[768]; bn = q[896];
+  };
   // window centred on cell f0-2 (slot 0 is never used): the loop below first shifts it
 #pragma unroll
   for (int s = 1; s < 2 * R + 1; s++) {
     Prim p = load_prim_half(Uh, g, idx + (long long)(s - R - 2) * sA);
     win[s] = to_W<A>(p, bnc[s]);
+    if (WSM) wput(s, win[s], bnc[s]);   // ring position of window slot s at "time" 0
   }
   win[0] = win[1]; bnc[0] = bnc[1];
+  if (WSM) wput(0, win[0], bnc[0]);
+  int ring = 0;  // ring slot that holds window slot 0
   W7 WL = win[1], lo, hi;
   F7 fprev;
   fprev.m = fprev.mn = fprev.mt1 = fprev.mt2 = fprev.e = fprev.by = fprev.bz = 0.0;
@@ -552,8 +570,10 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
   // cell is then reconstructed by the same instruction sequence, so mirror-image cells give
   // mirror-image states bit for bit.
   for (int f = f0 - 1; f <= fend; f++, idx += sA) {
+    if (!WSM) {
 #pragma unroll
-    for (int s = 0; s < 2 * R; s++) { win[s] = win[s + 1]; bnc[s] = bnc[s + 1]; }
+      for (int s = 0; s < 2 * R; s++) { win[s] = win[s + 1]; bnc[s] = bnc[s + 1]; }
+    }
     {
       Prim p;
       if (PREF) {
@@ -571,6 +591,15 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
       }
       win[2 * R] = to_W<A>(p, bnc[2 * R]);
       cp_async_commit();
+    }
+    if (WSM) {  // the oldest ring slot takes the new cell; the window is re-read slot by slot
+      wput(ring, win[2 * R], bnc[2 * R]);
+      ring = (ring + 1 == 5) ? 0 : ring + 1;
+#pragma unroll
+      for (int s = 0; s < 2 * R; s++) {
+        int slot = ring + s; slot = (slot >= 5) ? slot - 5 : slot;
+        wget(slot, win[s], bnc[s]);
+      }
     }
     reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
     if (f >= f0) {
