@@ -104,15 +104,11 @@ void extents(int f, const Geo &g, int &ex, int &ey, int &ez) {
 int fill_ghosts(State8 &U) {
   const Geo &g = C.g;
   const int B = 256;
-  long long t0 = 2LL * g.ng * g.N[1] * g.N[2];
-  k_fill_ghosts<0><<<dim3(grid1(t0, B).x, 1, NFIELD), B, 0, C.stream>>>(U, g);
-  LAUNCH_CHECK("k_fill_ghosts<0>");
-  long long t1 = 2LL * g.ng * g.N[0] * g.N[2];
-  k_fill_ghosts<1><<<dim3(grid1(t1, B).x, 1, NFIELD), B, 0, C.stream>>>(U, g);
-  LAUNCH_CHECK("k_fill_ghosts<1>");
-  long long t2 = 2LL * g.ng * g.N[0] * g.N[1];
-  k_fill_ghosts<2><<<dim3(grid1(t2, B).x, 1, NFIELD), B, 0, C.stream>>>(U, g);
-  LAUNCH_CHECK("k_fill_ghosts<2>");
+  const long long L0 = g.n[0] + 2 * g.ng, L1 = g.n[1] + 2 * g.ng;
+  long long t0 = L0 * L1 * 2 * g.ng, t1 = L0 * 2 * g.ng * g.n[2], t2 = 2LL * g.ng * g.n[1] * g.n[2];
+  long long tmax = t0 > t1 ? (t0 > t2 ? t0 : t2) : (t1 > t2 ? t1 : t2);
+  k_fill_ghosts<<<dim3(grid1(tmax, B).x, 3, NFIELD), B, 0, C.stream>>>(U, g);
+  LAUNCH_CHECK("k_fill_ghosts");
   return MHD_OK;
 }
 

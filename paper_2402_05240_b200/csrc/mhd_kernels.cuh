@@ -1,6 +1,6 @@
 // mhd_kernels.cuh -- the CUDA kernels of one VL+CT step, sm_100a, fp64.
 //
-//   k_fill_ghosts<AXIS>   a0  periodic / outflow ghost layers (O12)
+//   k_fill_ghosts         a0  periodic / outflow ghost layers (O12)
 //   k_cfl                 a1  Eq. 11-12 + warp-shuffle/block/atomic min
 //   k_predictor_flux      a2  PCM + HLLD on the three lower faces of a cell
 //   k_ct                  a3/a7  CT edge fields, Eq. 15-18
@@ -14,47 +14,47 @@
 namespace mhd {
 
 // ---------------------------------------------------------------------------------------
-// a0: ghost fill along one axis over the full raw extent of the other two (so edges and
-// corners are filled by the x, y, z sequence).  Thread = (ghost slot, p, q); blockIdx.z = field.
+// a0: ghost fill (O12), all three axes in one launch.  Filling x, then y, then z
+// over the full extent of the other two axes gives every ghost cell the value of the cell at
+// (src_x(i), src_y(j), src_z(k)), where src_a is the per-axis boundary map; this kernel applies the
+// composed map directly.  Periodic: src = i mod n (so the upper boundary face of the normal field
+// copies face 0).  Outflow: nearest active cell, or nearest active face 0..n for the normal field.
+// blockIdx.z = field; blockIdx.y = region: 0 = the z ghost slabs over all (i, j), 1 = the y ghost
+// slabs over all i and active k, 2 = the x ghost columns over active (j, k) -- disjoint, together
+// every index with at least one ghost coordinate.
 // ---------------------------------------------------------------------------------------
-template <int AXIS>
-__global__ void k_fill_ghosts(State8 U, Geo g) {
-  constexpr int A1 = (AXIS + 1) % 3, A2 = (AXIS + 2) % 3;
-  const int f = blockIdx.z;
-  const int ng = g.ng, na = g.n[AXIS];
-  // fastest thread index runs along x whenever x is not the fill axis
-  int e0, e1, e2;  // extents of (fast, mid, slow) loop
-  if (AXIS == 0) { e0 = 2 * ng; e1 = g.N[1]; e2 = g.N[2]; }
-  else if (AXIS == 1) { e0 = g.N[0]; e1 = 2 * ng; e2 = g.N[2]; }
-  else { e0 = g.N[0]; e1 = g.N[1]; e2 = 2 * ng; }
+__device__ __forceinline__ int ghost_src(int i, int n, int bc, bool normalB) {
+  if (bc == MHD_BC_PERIODIC) { int s = i % n; return s < 0 ? s + n : s; }
+  if (normalB) return i < 0 ? 0 : (i > n ? n : i);
+  return i < 0 ? 0 : (i >= n ? n - 1 : i);
+}
+
+__device__ __forceinline__ int ghost_slot(int slot, int ng, int n) {  // slot 0..2ng-1 -> logical index
+  return slot < ng ? slot - ng : n + (slot - ng);
+}
+
+__global__ void __launch_bounds__(256) k_fill_ghosts(State8 U, Geo g) {
+  const int f = blockIdx.z, region = blockIdx.y;
+  const int ng = g.ng, n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
+  const int L0 = n0 + 2 * ng, L1 = n1 + 2 * ng;
   long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  long long tot = (long long)e0 * e1 * e2;
-  if (t >= tot) return;
-  int c0 = (int)(t % e0);
-  int c1 = (int)((t / e0) % e1);
-  int c2 = (int)(t / ((long long)e0 * e1));
-  int slot, r1, r2;  // ghost slot along AXIS, raw positions along A1, A2
-  if (AXIS == 0) { slot = c0; r1 = c1; r2 = c2; }
-  else if (AXIS == 1) { slot = c1; r2 = c0; r1 = c2; }   // A1 = z, A2 = x
-  else { slot = c2; r1 = c0; r2 = c1; }                 // A1 = x, A2 = y
-  int i = (slot < ng) ? slot - ng : na + (slot - ng);   // logical index along AXIS
-  const bool normalB = (f == F_BX + AXIS);
-  int src;
-  if (g.bc[AXIS] == MHD_BC_PERIODIC) {
-    src = i % na;
-    if (src < 0) src += na;
+  int i, j, k;
+  if (region == 0) {
+    if (t >= (long long)L0 * L1 * 2 * ng) return;
+    i = (int)(t % L0) - ng; j = (int)((t / L0) % L1) - ng; k = ghost_slot((int)(t / ((long long)L0 * L1)), ng, n2);
+  } else if (region == 1) {
+    if (t >= (long long)L0 * 2 * ng * n2) return;
+    i = (int)(t % L0) - ng; j = ghost_slot((int)((t / L0) % (2 * ng)), ng, n1); k = (int)(t / ((long long)L0 * 2 * ng));
   } else {
-    if (normalB) {  // faces 0..na are active
-      if (i == na) return;
-      src = (i < 0) ? 0 : na;
-    } else {
-      src = (i < 0) ? 0 : na - 1;
-    }
+    if (t >= 2LL * ng * n1 * n2) return;
+    i = ghost_slot((int)(t % (2 * ng)), ng, n0); j = (int)((t / (2 * ng)) % n1); k = (int)(t / (2LL * ng * n1));
   }
-  const int off = (AXIS == 0) ? g.ox : ng;
-  long long base = (long long)r1 * g.s[A1] + (long long)r2 * g.s[A2];
+  const int si = ghost_src(i, n0, g.bc[0], f == F_BX);
+  const int sj = ghost_src(j, n1, g.bc[1], f == F_BY);
+  const int sk = ghost_src(k, n2, g.bc[2], f == F_BZ);
+  if (si == i && sj == j && sk == k) return;  // an active face of the normal field on an outflow side
   double *p = U.f[f];
-  p[base + (long long)(i + off) * g.s[AXIS]] = p[base + (long long)(src + off) * g.s[AXIS]];
+  p[cell_index(g, i, j, k)] = p[cell_index(g, si, sj, sk)];
 }
 
 // ---------------------------------------------------------------------------------------
