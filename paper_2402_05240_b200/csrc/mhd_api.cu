@@ -1,11 +1,13 @@
 // mhd_api.cu -- C ABI (include/mhd.h) of the B200 VL+CT ideal-MHD step: context, memory
 // carving, launch sequence of one step.  Pure CUDA runtime; no torch types.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <cuda_runtime.h>
 
 #include "../../include/mhd.h"
 #include "mhd_kernels.cuh"
+#include "mhd_stage.cuh"
 
 using namespace mhd;
 
@@ -33,6 +35,8 @@ struct Context {
   cudaGraphExec_t graph[2] = {nullptr, nullptr};  // one per orientation of the B ping-pong
   double graph_cfl[2] = {0.0, 0.0};
   long long graph_launches = 0;
+  int num_sms = 148;
+  int stage_ty = MHD_STAGE_TY;  // rows per block of the fused predictor stage (0 = three kernels)
   int parity = 0;  // flips with every step (which set of face arrays holds B^n)
   // per-launch event timing (mhd_step_profile)
   int prof_n = -1;  // -1 = off, else number of launches recorded so far
@@ -155,12 +159,36 @@ int launch_corrector_fluxes() {
 }
 
 // One VL+CT step with the dt held in C.sc->dt.
-int step_kernels() {
+// Steps 2-5 (PCM + HLLD on cells [-2-r, n+r+1], CT on indices [-1-r, n+r+1], half update of
+// cells [-1-r, n+r]).  MHD_STAGE_TY = 0 runs them as three kernels through the flux arrays,
+// otherwise as the single fused kernel of mhd_stage.cuh with TY rows per block.
+template <int TY>
+int launch_stage_kernel(const Box &hb) {
+  const Geo &g = C.g;
+  const int ntx = (hb.hi[0] - hb.lo[0] + 2 + 29) / 30, nty = (hb.hi[1] - hb.lo[1] + 2 + TY - 3) / (TY - 2);
+  const int nz = hb.hi[2] - hb.lo[2] + 1;
+  const long long tiles = (long long)ntx * nty;
+  const long long slots = (long long)C.num_sms * (TY <= 8 ? 2 : 1);
+  // z is cut into chunks so that the tiles fill the SMs in whole waves; every chunk pays two extra planes
+  int best = 1;
+  long long best_cost = -1;
+  for (int c = 1; c <= nz && c <= 64; c++) {
+    long long cost = ((tiles * c + slots - 1) / slots) * ((nz + c - 1) / c + 2);
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = c; }
+  }
+  const int lz = (nz + best - 1) / best;
+  const size_t smem = (size_t)MHD_STAGE_COLS * 32 * TY * sizeof(double);
+  k_predictor_stage<TY><<<dim3((unsigned)tiles, best), 32 * TY, smem, C.stream>>>(C.U, C.Uh, C.Er, g, hb, C.sc, ntx, lz);
+  LAUNCH_CHECK("k_predictor_stage");
+  return MHD_OK;
+}
+
+int launch_predictor_stage() {
   const Geo &g = C.g;
   const int r = recon_radius(g.recon);
-  int rc = fill_ghosts(C.U);  // one boundary update per step (PAPER.md:295)
-  if (rc) return rc;
-  // Steps 2-3: PCM + HLLD on cells [-2-r, n+r+1]
+  Box hb;
+  for (int a = 0; a < 3; a++) { hb.lo[a] = -1 - r; hb.hi[a] = g.n[a] + r; }
+  if (C.stage_ty == 12) return launch_stage_kernel<12>(hb);
   Box pb;
   for (int a = 0; a < 3; a++) { pb.lo[a] = -2 - r; pb.hi[a] = g.n[a] + r + 1; }
   {
@@ -169,9 +197,6 @@ int step_kernels() {
     k_predictor_flux<<<grid, 128, 0, C.stream>>>(C.U, C.F, C.Er, g, pb);
     LAUNCH_CHECK("k_predictor_flux");
   }
-  // Step 4: CT on indices [-1-r, n+r+1];  Step 5: half update of cells [-1-r, n+r]
-  Box hb;
-  for (int a = 0; a < 3; a++) { hb.lo[a] = -1 - r; hb.hi[a] = g.n[a] + r; }
   {
     Box eb = hb;
     for (int a = 0; a < 3; a++) eb.hi[a] += 1;
@@ -183,6 +208,16 @@ int step_kernels() {
     k_update<true><<<gridu, 256, 0, C.stream>>>(C.U, C.Uh, C.F, C.E, C.Er, g, hb, C.sc, 0.5);
     LAUNCH_CHECK("k_update(half)");
   }
+  return MHD_OK;
+}
+
+int step_kernels() {
+  const Geo &g = C.g;
+  const int r = recon_radius(g.recon);
+  int rc = fill_ghosts(C.U);  // one boundary update per step (PAPER.md:295)
+  if (rc) return rc;
+  rc = launch_predictor_stage();
+  if (rc) return rc;
   // Steps 6-7: reconstruction + HLLD from U^{n+1/2}
   switch (g.recon) {
     case 0: rc = launch_corrector_fluxes<0>(); break;
@@ -281,6 +316,16 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
   }
   Geo g;
   if (!make_geo(g, nx, ny, nz, gamma, recon)) return fail(MHD_ERR_ARG, "mhd_init: bad argument");
+  {
+    const int cols = MHD_STAGE_COLS * 32 * (int)sizeof(double);
+    CU(cudaFuncSetAttribute(k_predictor_stage<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols * 12));
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    C.num_sms = sms > 0 ? sms : 148;
+    const char *e = getenv("MHD_STAGE_TY");
+    if (e) C.stage_ty = atoi(e);
+  }
   size_t need = total_bytes(g);
   if (ws) {
     if (ws_bytes < need || ((size_t)ws & 255)) return fail(MHD_ERR_NOMEM, "workspace too small or misaligned");
