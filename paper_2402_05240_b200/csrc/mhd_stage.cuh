@@ -166,11 +166,7 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
       Fx0 = f.m; Fx6 = f.bz;
     }
     double Fyh[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-#ifdef MHD_STAGE_YALL
-    {
-#else
     if (row > 0) {  // y face (the lowest row only lends its x and z faces)
-#endif
       F7 f = stage_face<1>(g, prim_fetch<NT>(P, td), pc, byl);
       Fyh[0] = f.m; Fyh[1] = f.mn; Fyh[2] = f.mt1; Fyh[3] = f.mt2; Fyh[4] = f.e;
       Fy5 = f.by; Fy6 = f.bz;
