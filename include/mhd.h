@@ -57,7 +57,10 @@ size_t mhd_workspace_bytes(int nx, int ny, int nz, int recon);
 /* Create the context (the nine-step VL+CT list): nx*ny*nz cells on the unit
  * box, adiabatic index gamma > 1, recon one of MHD_RECON_*.  All axes periodic
  * until mhd_set_boundary says otherwise.  Device memory is obtained with cudaMalloc.
- * A previous context is destroyed first. */
+ * A previous context is destroyed first.
+ * Developer switch: if the environment variable MHD_STAGE_TY is "0" when the context is created,
+ * the predictor stage (steps 2-5 of the list) runs as three kernels through the flux arrays instead
+ * of the single fused kernel (same arithmetic, results equal to rounding; slower). */
 int mhd_init(int nx, int ny, int nz, double gamma, int recon);
 
 /* Same, but all device arrays are carved out of `workspace` (a DEVICE pointer, 256-byte
