@@ -46,10 +46,18 @@ KERNEL_MODEL = {
     "k_ct(corrector)":        (77, (9 + 3 + 3) * 8),            # mass/magnetic fluxes + E_ref -> edge E
     "k_update(B)+cfl":        (191, (3 + 3 + 5 + 3) * 8),       # B^n, edge E, U^{n+1} hydro -> B^{n+1}; CFL rate
 }
-# dram__bytes_read.sum + dram__bytes_write.sum per launch (GB) from the same ncu capture
-NCU_TRAFFIC_GB = {"k_predictor_stage": 2.77, "k_flux_x": 2.07, "k_flux_march<1>": 2.11,
-                  "k_flux_march<2>+update": 4.33, "k_ct(corrector)": 2.09, "k_update(B)+cfl": 1.93}
-STEP_FLOP_PER_CELL = sum(v[0] for v in KERNEL_MODEL.values())     # 4310 (PLMC), algorithmic
+# the same for PPMC (ncu capture of `--workload 256:ppmc`, profiles/r1_ncu_kernels.md): only the sweeps differ
+KERNEL_MODEL_PPMC = dict(KERNEL_MODEL)
+KERNEL_MODEL_PPMC.update({"k_flux_x": (1068, (8 + 7) * 8), "k_flux_march<1>": (1057, (8 + 7) * 8),
+                          "k_flux_march<2>+update": (1121, (8 + 3 + 5 + 10 + 5) * 8),
+                          "k_ct(corrector)": (76, (9 + 3 + 3) * 8), "k_update(B)+cfl": (190, (3 + 3 + 5 + 3) * 8)})
+MODELS = {1: KERNEL_MODEL, 2: KERNEL_MODEL_PPMC}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (GB) from the same ncu captures (256^3)
+NCU_TRAFFIC_GB = {1: {"k_predictor_stage": 2.77, "k_flux_x": 2.07, "k_flux_march<1>": 2.11,
+                      "k_flux_march<2>+update": 4.33, "k_ct(corrector)": 2.09, "k_update(B)+cfl": 1.93},
+                  2: {"k_predictor_stage": 2.85, "k_flux_x": 2.11, "k_flux_march<1>": 2.20,
+                      "k_flux_march<2>+update": 4.52, "k_ct(corrector)": 2.14, "k_update(B)+cfl": 1.98}}
+STEP_FLOP_PER_CELL = sum(v[0] for v in KERNEL_MODEL.values())     # 4310 (PLMC; PPMC 4900), algorithmic
 STEP_BYTES_PER_CELL = sum(v[1] for v in KERNEL_MODEL.values())    # 872 as materialised; floor 128
 
 
@@ -325,15 +333,16 @@ def run_b200(args):
     if rank == 0:
         hbm_peak, hbm_src = load_measured_peaks()
         step_ms = sum(prof.values())
+        model = MODELS.get(p.recon)   # FLOP counts were taken on the PLMC and PPMC builds
         top = max((k for k in prof if k in KERNEL_MODEL), key=lambda k: prof[k])
-        flop_cell, byte_cell = KERNEL_MODEL[top]
-        if p.recon != 1:
-            flop_cell = None  # FLOP counts were taken on the PLMC build only
+        flop_cell, byte_cell = (model or KERNEL_MODEL)[top]
+        if model is None:
+            flop_cell = None
         t_top = prof[top] * 1e-3
-        traffic = NCU_TRAFFIC_GB.get(top) if (tuple(p.n) == (256, 256, 256) and p.recon == 1) else None
+        traffic = NCU_TRAFFIC_GB[p.recon].get(top) if (tuple(p.n) == (256, 256, 256) and model) else None
         roof = {"kernel": top, "kernel_ms": prof[top], "share_of_step": prof[top] / step_ms,
                 "traffic": traffic * 1e9 if traffic else None,
-                "traffic_source": "profiles/r1_ncu_kernels.md (ncu --set full, 256^3 PLMC)" if traffic else None}
+                "traffic_source": "profiles/r1_ncu_kernels.md (ncu --set full, 256^3)" if traffic else None}
         hbm_ach = byte_cell * nc / t_top / 1e9
         roof["algorithmic_bytes_per_launch"] = byte_cell * nc
         if flop_cell is not None and flop_cell * nc / (fp64_tf * 1e12) > byte_cell * nc / (hbm_peak * 1e9):
@@ -348,18 +357,19 @@ def run_b200(args):
                 roof["fp64_achieved_tflops"] = flop_cell * nc / t_top / 1e12
         # whole-step roofline (north_star): the slower of counted FLOPs at the measured fp64 peak and
         # the bytes the design moves at the measured HBM bandwidth; the 128 B/cell floor beside it
-        if p.recon == 1:
-            t_flop = STEP_FLOP_PER_CELL * nc / (fp64_tf * 1e12)
+        if model:
+            step_flop = sum(v[0] for v in model.values())
+            t_flop = step_flop * nc / (fp64_tf * 1e12)
             t_byte = STEP_BYTES_PER_CELL * nc / (hbm_peak * 1e9)
             t_step = ms / args.steps * 1e-3 / 1.0
             # kernels run one after another, each against its own bound: sum of max(flop, bytes) times
-            t_serial = sum(max(fc * nc / (fp64_tf * 1e12), bc * nc / (hbm_peak * 1e9)) for fc, bc in KERNEL_MODEL.values())
-            roof["step"] = {"flop_per_cell": STEP_FLOP_PER_CELL, "bytes_per_cell": STEP_BYTES_PER_CELL,
+            t_serial = sum(max(fc * nc / (fp64_tf * 1e12), bc * nc / (hbm_peak * 1e9)) for fc, bc in model.values())
+            roof["step"] = {"flop_per_cell": step_flop, "bytes_per_cell": STEP_BYTES_PER_CELL,
                             "t_flop_ms": t_flop * 1e3, "t_bytes_ms": t_byte * 1e3,
                             "frac_of_roofline": max(t_flop, t_byte) / t_step,
                             "t_serial_ms": t_serial * 1e3, "frac_of_serial_roofline": t_serial / t_step,
                             "frac_of_128B_floor": (128.0 * nc / (hbm_peak * 1e9)) / t_step,
-                            "fp64_tflops_step": STEP_FLOP_PER_CELL * nc / t_step / 1e12}
+                            "fp64_tflops_step": step_flop * nc / t_step / 1e12}
         roof["kernels_ms"] = {k: round(v, 4) for k, v in prof.items()}
         roof["measured_here"] = {"fp64_tflops": fp64_tf, "copy_gbs": copy_gbs}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
