@@ -38,7 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if res.returncode:
         raise RuntimeError("nvcc failed: %s" % " ".join(cmd))
     with open(os.path.join(HERE, "ptxas_info.txt"), "w") as fh:
-        fh.write("# " + " ".join(cmd) + "\n" + res.stdout)
+        # (compile times left out: they change from run to run and would dirty the tracked file)
+        fh.write("# " + " ".join(cmd) + "\n" + "".join(l for l in res.stdout.splitlines(True) if "Compile time" not in l))
     return LIB
 
 
