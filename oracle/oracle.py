@@ -52,6 +52,8 @@ def lib():
         L.oracle_phys_flux.argtypes = [_d, _dp, _d, _dp]
         L.oracle_phys_flux.restype = None
         L.oracle_num_threads.restype = ctypes.c_int
+        L.oracle_set_guards.argtypes = [ctypes.c_int, ctypes.c_int]
+        L.oracle_set_guards.restype = None
         _lib = L
     return _lib
 
@@ -127,6 +129,11 @@ def ct_edge(*args):
 
 def fast_speed(gamma, rho, P, bn, bt1, bt2):
     return lib().oracle_fast_speed(gamma, rho, P, bn, bt1, bt2)
+
+
+def set_guards(r6=True, r7=True):
+    """Pin support only: switch the round-off guards of readings R6 / R7 (both on by default)."""
+    lib().oracle_set_guards(int(bool(r6)), int(bool(r7)))
 
 
 def num_threads():

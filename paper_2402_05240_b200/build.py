@@ -20,6 +20,9 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 
 
+PTXAS_LOG = ""
+
+
 def nvcc():
     for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
         if cand and (os.path.isabs(cand) and os.path.exists(cand) or not os.path.isabs(cand)):
@@ -37,9 +40,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         print(res.stdout)
     if res.returncode:
         raise RuntimeError("nvcc failed: %s" % " ".join(cmd))
-    with open(os.path.join(HERE, "ptxas_info.txt"), "w") as fh:
-        # (compile times left out: they change from run to run and would dirty the tracked file)
-        fh.write("# " + " ".join(cmd) + "\n" + "".join(l for l in res.stdout.splitlines(True) if "Compile time" not in l))
+    global PTXAS_LOG
+    PTXAS_LOG = res.stdout   # registers / spills / shared memory per kernel (-Xptxas -v); nothing is written
     return LIB
 
 

@@ -26,6 +26,7 @@ struct Context {
   Edge3 E;   // CT edge fields
   Edge3 Er;  // cell-centred reference field, Eq. 18
   Edge3 Bnext;  // face arrays that receive B^{n+1}; swapped with U's after every step
+  double *scratch = nullptr;  // staging of the host set/get calls (never a result array)
   Scalars *sc = nullptr;
   cudaStream_t stream = 0;
   long long launches = 0;
@@ -93,7 +94,7 @@ bool make_geo(Geo &g, int nx, int ny, int nz, double gamma, int recon) {
   return true;
 }
 
-const int kNumArrays = 2 * NFIELD + 21 + 3 + 3 + 3;  // U, half state, fluxes, edge fields, reference field, B^{n+1}
+const int kNumArrays = 2 * NFIELD + 21 + 3 + 3 + 3 + 1;  // U, half state, fluxes, edge fields, reference field, B^{n+1}, scratch
 
 size_t array_bytes(const Geo &g) { return ((size_t)g.ntot * sizeof(double) + 255) / 256 * 256; }
 
@@ -347,6 +348,7 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
   for (int a = 0; a < 3; a++) { C.E.f[a] = (double *)p; p += ab; }
   for (int a = 0; a < 3; a++) { C.Er.f[a] = (double *)p; p += ab; }
   for (int a = 0; a < 3; a++) { C.Bnext.f[a] = (double *)p; p += ab; }
+  C.scratch = (double *)p; p += ab;
   C.launches = 0;
   C.rate_valid = false;
   C.inited = true;
@@ -366,8 +368,8 @@ int set_state_from(const double *const src[NFIELD], bool host) {
     extents(f, g, ex, ey, ez);
     long long cnt = (long long)ex * ey * ez;
     const double *dsrc = src[f];
-    if (host) {  // stage through a flux array (free between steps)
-      double *stage = C.F.f[f / 7][f % 7];
+    if (host) {  // staged through the scratch array; stream order keeps the fields apart
+      double *stage = C.scratch;
       CU(cudaMemcpyAsync(stage, src[f], cnt * sizeof(double), cudaMemcpyHostToDevice, C.stream));
       dsrc = stage;
     }
@@ -385,7 +387,7 @@ int get_state_to(State8 &S, double *const dst[NFIELD], bool host) {
     int ex, ey, ez;
     extents(f, g, ex, ey, ez);
     long long cnt = (long long)ex * ey * ez;
-    double *ddst = host ? C.F.f[f / 7][f % 7] : dst[f];
+    double *ddst = host ? C.scratch : dst[f];
     k_pack<<<grid1(cnt, 256), 256, 0, C.stream>>>(ddst, S.f[f], g, ex, ey, ez);
     LAUNCH_CHECK("k_pack");
     if (host) CU(cudaMemcpyAsync(dst[f], ddst, cnt * sizeof(double), cudaMemcpyDeviceToHost, C.stream));
@@ -543,10 +545,10 @@ int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *
   if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
   double *dst[NFIELD] = {rho, mx, my, mz, E, bx, by, bz};
   // the half state is held as (rho, v, P, face B): convert to the ABI's conserved variables in
-  // scratch (x-flux arrays 0..4 are free after the step; get_state_to stages through others)
+  // arrays that are dead after the step and exposed by no call (edge fields, B^n's old set)
   const Geo &g = C.g;
   State8 tmp = C.Uh;
-  for (int f = 0; f < 5; f++) tmp.f[f] = C.F.f[2][f];
+  tmp.f[0] = C.E.f[0]; tmp.f[1] = C.E.f[1]; tmp.f[2] = C.E.f[2]; tmp.f[3] = C.Bnext.f[0]; tmp.f[4] = C.Bnext.f[1];
   Box ab = make_box(0, g.n[0] - 1, 0, g.n[1] - 1, 0, g.n[2] - 1);
   long long plane = (long long)g.n[0] * g.n[1];
   k_half_to_cons<<<dim3(grid1(plane, 256).x, g.n[2]), 256, 0, C.stream>>>(C.Uh, tmp, g, ab);
@@ -564,7 +566,7 @@ int mhd_get_flux(int axis, int comp, double *out) {
     return fail(MHD_ERR_ARG, "mhd_get_flux: the z momentum / energy fluxes are consumed in the z sweep, not stored");
   const Geo &g = C.g;
   long long cnt = (long long)g.n[0] * g.n[1] * g.n[2];
-  double *stage = C.Uh.f[0];  // the half-step state is dead after the step
+  double *stage = C.scratch;
   k_pack<<<grid1(cnt, 256), 256, 0, C.stream>>>(stage, C.F.f[axis][comp], g, g.n[0], g.n[1], g.n[2]);
   LAUNCH_CHECK("k_pack");
   CU(cudaMemcpyAsync(out, stage, cnt * sizeof(double), cudaMemcpyDeviceToHost, C.stream));

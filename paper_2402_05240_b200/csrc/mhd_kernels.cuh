@@ -151,7 +151,9 @@ __global__ void __launch_bounds__(256) k_cfl(State8 U, Geo g, Scalars *sc) {
   block_rate_reduce(r, bad, sc);
 }
 
-__global__ void k_reset_rate(Scalars *sc) { sc->rate_bits = 0ull; }
+// new state (mhd_set_state, mhd_set_domain): the running maximum and the non-physical-state flag
+// belong to the state they were computed on
+__global__ void k_reset_rate(Scalars *sc) { sc->rate_bits = 0ull; sc->bad = 0ull; }
 
 // dt = cfl / max rate; accumulate time; re-arm the reduction
 __global__ void k_finish_dt(Scalars *sc, double cfl) {
@@ -177,7 +179,7 @@ __device__ __forceinline__ void store_eref(const Edge3 &Er, long long idx, const
 // reconstruction at no cost in registers.
 __device__ __forceinline__ void cp_async8(double *smem, const double *gmem) {
   unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem));
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -534,10 +536,12 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
     win[s] = to_W<A>(p, bnc[s]);
     if (WSM) wput(s, win[s], bnc[s]);   // ring position of window slot s at "time" 0
   }
-  win[0] = win[1]; bnc[0] = bnc[1];
+  if constexpr (R > 0) { win[0] = win[1]; bnc[0] = bnc[1]; }
   if (WSM) wput(0, win[0], bnc[0]);
   int ring = 0;  // ring slot that holds window slot 0
-  W7 WL = win[1], lo, hi;
+  W7 WL, lo, hi;
+  if constexpr (R > 0) WL = win[1];
+  else WL.rho = WL.u = WL.v = WL.w = WL.P = WL.by = WL.bz = 0.0;  // (replaced before its first use)
   F7 fprev;
   fprev.m = fprev.mn = fprev.mt1 = fprev.mt2 = fprev.e = fprev.by = fprev.bz = 0.0;
   // staging column of this thread: slots 0..4 = U (rho, mx, my, mz, E) of the cell to update,

@@ -379,6 +379,53 @@ def test_error_codes(mhd):
     g.close()
 
 
+def test_unphysical_flag_belongs_to_the_state_it_was_computed_on(mhd):
+    """MHD_ERR_UNPHYSICAL is not sticky: after a bad state, mhd_set_state(good) + mhd_compute_dt
+    succeeds (PAPER.md:523 on error reporting; SURVEY.md 8(b) error convention)."""
+    p = inputs.random_smooth(n=(12, 10, 8), seed=21)
+    bad = {k: v.copy() for k, v in p.state.items()}
+    bad["E"][3, 2, 1] = 0.0
+    g = mhd.Mhd(*p.n, p.gamma, 1)
+    g.set_state(bad)
+    with pytest.raises(mhd.MhdError):
+        g.compute_dt(0.4)
+    g.set_state(p.state)
+    o = orc.Oracle(*p.n, p.gamma, 1)
+    o.set_state(p.state)
+    dt = g.compute_dt(0.4)
+    assert abs(dt - o.compute_dt(0.4)) <= 1e-13 * dt
+    g.step(dt)
+    assert g.compute_dt(0.4) > 0.0          # the flag of the new state, folded into the full update
+    assert g.advance(2, 0.4, want_time=True) > 0.0
+    g.close(); o.close()
+
+
+@pytest.mark.timeout(1800)
+def test_full_size_256_cube_ten_steps(mhd):
+    """BASELINE.json configs[2] as stated: 256^3, 10 steps.  Every step is a one-step parity case
+    from the oracle's own state, every cell (1e-12), and the free-running GPU state after the 10
+    steps (mhd_advance, the call bench.py times) is compared with the oracle's at the run bound."""
+    p = inputs.turbulence(256, n_steps=10)
+    o, g = make_pair(mhd, p)
+    state = p.state
+    for s in range(p.n_steps):
+        if s:
+            g.set_state(state)
+        dt = o.compute_dt(p.cfl)
+        assert abs(g.compute_dt(p.cfl) - dt) <= 1e-13 * dt
+        o.step(dt); g.step(dt)
+        state = o.get_state()
+        out = g.get_state()
+        assert_close(out, state, TOL_STEP, "256^3 step %d" % (s + 1))
+        assert divb_normalised(out, p.n) <= TOL_DIVB
+    g.set_state(p.state)
+    g.advance(p.n_steps, p.cfl)
+    out = g.get_state()
+    assert_close(out, state, TOL_RUN, "256^3 ten free-running steps")
+    assert divb_normalised(out, p.n) <= TOL_DIVB
+    o.close(); g.close()
+
+
 @pytest.mark.timeout(900)
 def test_full_size_256_cube_one_step(mhd):
     """BASELINE.json configs[2] at full size (256^3, the bench workload and launch configuration):

@@ -235,13 +235,10 @@ def test_T13_blast_symmetry_and_positivity():
     # Point symmetry about the box centre (rho, E even; m odd; B even -- B is axial) and, with B
     # along (1,1,1), invariance under the cyclic permutation x->y->z.  The scheme itself is
     # symmetric to round-off on generic data (test_inversion_symmetry_generic_state).  On the blast
-    # the cell fields are symmetric to round-off after the first step, but the upwind switch of
-    # Eq. 16 ("v>0 / v<0 / otherwise") acts on mass fluxes that are zero up to
-    # round-off near the centre, and flips between mirror-image edges; the difference between its
-    # branches is a truncation-level quantity, so a handful of faces differ at ~1e-3 at once and
-    # the asymmetry then spreads at ~1e-4..1e-2 of the blast amplitude.
-    # That is a property of the published algorithm, not pinned here
-    # beyond a loose bound.
+    # the upwind switch of Eq. 16 ("v>0 / v<0 / otherwise") acts on mass fluxes
+    # that are zero analytically near the centre; reading R6 makes HLLD return exactly
+    # zero there, the "otherwise" branch is taken on both mirror images, and EVERY face stays
+    # symmetric to round-off (tests/test_oracle_guards.py shows what happens without it).
     inv = lambda a: a[::-1, ::-1, ::-1]
     for recon in (1, 2):
         p = inputs.blast(n=24, n_steps=12, recon=recon)
@@ -252,11 +249,11 @@ def test_T13_blast_symmetry_and_positivity():
         assert np.max(np.abs(st["E"] - inv(st["E"]))) < 1e-13
         for f in ("mx", "my", "mz"):
             assert np.max(np.abs(st[f] + inv(st[f]))) < 1e-14
-        # B: symmetric except on the few faces next to edges whose mass flux is zero up to
-        # round-off (24 of 14400 per component at n=24) -- the Eq. 16 switch, see above
-        for f in ("bx", "by", "bz"):
-            bad = np.abs(st[f] - inv(st[f])) > 1e-13
-            assert bad.sum() <= 0.005 * bad.size, (recon, f, int(bad.sum()))
+        # B lives on the lower faces: face f of the inverted grid is face n - f
+        for f, ax in (("bx", 2), ("by", 1), ("bz", 0)):
+            a = st[f]
+            img = np.flip(a, axis=(0, 1, 2))
+            assert int((np.abs(a - img) > 1e-13).sum()) == 0, (recon, f)
         assert np.max(np.abs(st["rho"] - np.transpose(st["rho"], (1, 2, 0)))) < 1e-14
         assert np.max(np.abs(st["mx"] - np.transpose(st["mz"], (1, 2, 0)))) < 1e-14
         run_steps(o, p, p.n_steps - 1)
