@@ -426,21 +426,6 @@ def test_full_size_256_cube_ten_steps(mhd):
     o.close(); g.close()
 
 
-@pytest.mark.timeout(900)
-def test_full_size_256_cube_one_step(mhd):
-    """BASELINE.json configs[2] at full size (256^3, the bench workload and launch configuration):
-    one step against the oracle, every cell."""
-    p = inputs.turbulence(256, n_steps=1)
-    o, g = make_pair(mhd, p)
-    dt = o.compute_dt(p.cfl)
-    assert abs(g.compute_dt(p.cfl) - dt) <= 1e-13 * dt
-    o.step(dt); g.step(dt)
-    out = g.get_state()
-    assert_close(out, o.get_state(), TOL_STEP, "256^3 one step")
-    assert divb_normalised(out, p.n) <= TOL_DIVB
-    o.close(); g.close()
-
-
 def _sub_box(state, org, m):
     """m^3 cells of a full-size state starting at org = (i0, j0, k0), in the ABI layout of an m^3 grid."""
     i0, j0, k0 = org
