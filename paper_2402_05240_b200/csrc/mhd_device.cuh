@@ -36,136 +36,162 @@ __device__ __forceinline__ double fast_speed_sq(double gamma, double irho, doubl
 
 // ---------------------------------------------------------------------------------------
 // HLLD (Miyoshi & Kusano 2005, cited PAPER.md:149; reading O4, wave speeds G15).
-// Work is kept to what the selected branch needs: total pressure / energy of both sides and both
-// single-star states always (S_M, p_T* and the double-star state need them), the physical flux
-// only of the side that bounds the face.  Seven reciprocals and three square roots per solve.
+//
+// The flux in every region of the fan is evaluated as the physical flux function of that region's
+// state with the fan's total pressure p_T* in place of p_T:
+//     F*_a = F_a + S_a (U*_a - U_a)            == Eq. 8 applied to (rho*, S_M, v*, w*, B*, e*; p_T*)
+//     F**_a = F*_a + S*_a (U**_a - U*_a)       == Eq. 8 applied to (rho*, S_M, v**, w**, B**, e**; p_T*)
+// These are identities, not approximations: U*_a is DEFINED by the jump conditions across S_a
+// (M&K Eq. 43-48) and U** by those across S*_a (Eq. 59-63).  The one exception is M&K's degenerate
+// case (|D| < eps p_T*: the tangential components are left unchanged, which is not a solution of the
+// jump conditions for B_t): there F_a + S_a (U*_a - U_a) has the extra terms B_t,a (u_a - S_M) in
+// the two induction components, which are added explicitly.  One flux evaluation instead of three,
+// only the side that bounds the face gets its energy, the other side's star state is formed only
+// where the double-star state is needed, and no reciprocal of rho_L, rho_R is taken at all
+// (the larger fast speed is found by cross-multiplication).  ~200 fp64 instructions per solve.
 // ---------------------------------------------------------------------------------------
-struct HlldSide {
-  double rho, u, v, w, by, bz;        // primitive inputs
-  double pT, e;                       // total pressure, total energy density
-  double rhos, vs, ws, bys, bzs;      // single-star state (its energy is formed for one side only)
-  double Su, iSSm;                    // S - u, 1 / (S - S_M)
-};
-
-__device__ __forceinline__ void hlld_side_init(HlldSide &s, const W7 &W, double bx, double gm1inv) {
-  s.rho = W.rho; s.u = W.u; s.v = W.v; s.w = W.w; s.by = W.by; s.bz = W.bz;
-  double b2 = bx * bx + W.by * W.by + W.bz * W.bz;
-  s.pT = W.P + 0.5 * b2;
-  s.e = W.P * gm1inv + 0.5 * W.rho * (W.u * W.u + W.v * W.v + W.w * W.w) + 0.5 * b2;
+__device__ __forceinline__ int hi32(double x) { return __double2hiint(x); }
+__device__ __forceinline__ double xor_sign(double x, int signbit) {
+  return __hiloint2double(__double2hiint(x) ^ signbit, __double2loint(x));
 }
 
-// Eq. 8 without the zero row
-__device__ __forceinline__ F7 phys_flux(const HlldSide &s, double bx) {
+// x, or +tiny where x is negative, zero or denormal (round-off guard R3 of the discriminant of
+// Eq. 12: it is >= 0 analytically; 2^-1000 keeps the seed instruction of the root off 0)
+__device__ __forceinline__ double floor_tiny(double x) { return (hi32(x) < 0x00100000) ? 0x1p-1000 : x; }
+
+struct HlldSide {
+  double rho, u, v, w, P, by, bz;
+  double hb2, pT;   // B^2 / 2, total pressure
+  double X;         // gamma P + B^2 + sqrt(disc) = 2 rho c_f^2   (Eq. 12)
+};
+
+__device__ __forceinline__ void hlld_side_init(HlldSide &s, const W7 &W, double gamma, double bx2, double bx2x4) {
+  s.rho = W.rho; s.u = W.u; s.v = W.v; s.w = W.w; s.P = W.P; s.by = W.by; s.bz = W.bz;
+  double b2 = (W.by * W.by + W.bz * W.bz) + bx2;
+  s.hb2 = 0.5 * b2;
+  s.pT = W.P + s.hb2;
+  double gp = gamma * W.P;
+  double sm = gp + b2;
+  double disc = floor_tiny(sm * sm - gp * bx2x4);
+  s.X = sm + sqrt_nz(disc);
+}
+
+// Eq. 8 without the zero row, for the state (rho, u, v, w, by, bz, e) under the
+// total pressure pT; vb = u bx + v by + w bz
+__device__ __forceinline__ F7 flux_of(double rho, double u, double v, double w, double by, double bz, double e,
+                                      double pT, double vb, double bx, double bx2) {
   F7 F;
-  double ru = s.rho * s.u;
-  F.m = ru;
-  F.mn = ru * s.u + s.pT - bx * bx;
-  F.mt1 = ru * s.v - bx * s.by;
-  F.mt2 = ru * s.w - bx * s.bz;
-  F.e = s.u * (s.e + s.pT) - bx * (s.u * bx + s.v * s.by + s.w * s.bz);
-  F.by = s.by * s.u - bx * s.v;
-  F.bz = s.bz * s.u - bx * s.w;
+  double m = rho * u;
+  F.m = m;
+  F.mn = m * u + (pT - bx2);
+  F.mt1 = m * v - bx * by;
+  F.mt2 = m * w - bx * bz;
+  F.e = u * (e + pT) - bx * vb;
+  F.by = by * u - bx * v;
+  F.bz = bz * u - bx * w;
   return F;
 }
 
-// single-star state of one side (M&K Eq. 43-48); S = outer speed of this side
-__device__ __forceinline__ void hlld_star(HlldSide &s, double S, double SM, double pTs, double bx) {
-  double Su = S - s.u;
-  double SSm = S - SM;
-  double D = s.rho * Su * SSm - bx * bx;
-  double iSSm;
-  if (fabs(D) < 1e-8 * pTs) {  // degenerate 0/0: no jump in the tangential fields
-    iSSm = rcp(SSm);
-    s.vs = s.v; s.ws = s.w; s.bys = s.by; s.bzs = s.bz;
-  } else {
-    double inv = rcp(D * SSm);  // one reciprocal for 1/D and 1/(S - S_M)
-    double iD = inv * SSm;
-    iSSm = inv * D;
-    double fv = bx * (SM - s.u) * iD;
-    double fb = (s.rho * Su * Su - bx * bx) * iD;
-    s.vs = s.v - s.by * fv;
-    s.ws = s.w - s.bz * fv;
-    s.bys = s.by * fb;
-    s.bzs = s.bz * fb;
-  }
-  s.rhos = s.rho * (Su * iSSm);
-  s.Su = Su; s.iSSm = iSSm;
+__device__ __forceinline__ double total_energy(double gm1inv, double rho, double u, double v, double w, double P,
+                                               double hb2) {
+  return (0.5 * rho) * (u * u + v * v + w * w) + (P * gm1inv + hb2);
 }
 
-// irL, irR = 1/rho of the two states (the callers have them or form them once)
-__device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, const W7 &WR, double irL,
-                                   double irR, double bx) {
+// single-star state of one side (M&K Eq. 43-47): S = outer speed, sdu = rho (S - u), dua = S_M - u.
+// With g = (S_M - u) / D:  v* = v - B_y B_x g,  B_y* = B_y + B_y rho (S - u) g   (the same as
+// M&K's (rho (S-u)^2 - B_x^2) / D, written as 1 + ...), so the degenerate case is g = 0.
+struct Star {
+  double rhos, vs, ws, bys, bzs, iSSm;
+  bool degen;
+};
+
+__device__ __forceinline__ Star hlld_star(double S, double SM, double sdu, double dua, double v, double w,
+                                          double by, double bz, double pTs, double bx, double bx2) {
+  Star q;
+  const double SSm = S - SM;
+  const double D = sdu * SSm - bx2;
+  q.degen = fabs(D) < 1e-8 * pTs;                // degenerate 0/0: no jump in the tangential fields
+  const double t = q.degen ? 1.0 : D;
+  const double inv = rcp(t * SSm);               // one reciprocal for 1/D and 1/(S - S_M)
+  q.iSSm = inv * t;
+  const double g = q.degen ? 0.0 : (inv * SSm) * dua;
+  const double fv = bx * g, fb = sdu * g;
+  q.vs = v - by * fv;
+  q.ws = w - bz * fv;
+  q.bys = by + by * fb;
+  q.bzs = bz + bz * fb;
+  q.rhos = sdu * q.iSSm;
+  return q;
+}
+
+__device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, const W7 &WR, double bx) {
+  const double bx2 = bx * bx, bx2x4 = 4.0 * bx2;
   HlldSide L, R;
-  hlld_side_init(L, WL, bx, gm1inv);
-  hlld_side_init(R, WR, bx, gm1inv);
-  double cf2L = fast_speed_sq(gamma, irL, WL.P, bx, L.by, L.bz);
-  double cf2R = fast_speed_sq(gamma, irR, WR.P, bx, R.by, R.bz);
-  double cfmax = sqrt_(fmax(cf2L, cf2R));
-  double SL = fmin(L.u, R.u) - cfmax;
-  double SR = fmax(L.u, R.u) + cfmax;
+  hlld_side_init(L, WL, gamma, bx2, bx2x4);
+  hlld_side_init(R, WR, gamma, bx2, bx2x4);
+  // G15: S_L = min(u_L, u_R) - max(c_fL, c_fR), S_R = max(u_L, u_R) + max(c_fL, c_fR), with
+  // c_f^2 = X / (2 rho): the larger one by cross-multiplication, its root as X rsqrt(2 rho X)
+  const bool lbig = L.X * R.rho > R.X * L.rho;
+  const double Xw = lbig ? L.X : R.X, rw = lbig ? L.rho : R.rho;
+  const double cfmax = Xw * rsqrt_((2.0 * rw) * Xw);
+  const bool ul = L.u < R.u;
+  const double SL = (ul ? L.u : R.u) - cfmax;
+  const double SR = (ul ? R.u : L.u) + cfmax;
 
-  if (SL > 0.0) return phys_flux(L, bx);
-  if (SR < 0.0) return phys_flux(R, bx);
-
-  // middle wave and total pressure of the fan (M&K Eq. 38, 41)
-  double sduL = (SL - L.u) * L.rho;
-  double sduR = (SR - R.u) * R.rho;
-  double iden = rcp(sduR - sduL);
-  double SM = (sduR * R.u - sduL * L.u - R.pT + L.pT) * iden;
-  double pTs = (sduR * L.pT - sduL * R.pT + L.rho * R.rho * (SR - R.u) * (SL - L.u) * (R.u - L.u)) * iden;
-
-  hlld_star(L, SL, SM, pTs, bx);
-  hlld_star(R, SR, SM, pTs, bx);
-  double rL, rR, irsL, irsR;
-  sqrt_rsqrt(L.rhos, rL, irsL);
-  sqrt_rsqrt(R.rhos, rR, irsR);
-  double abx = fabs(bx);
-  double SsL = SM - abx * irsL;
-  double SsR = SM + abx * irsR;
-
-  // side whose states bound the face: left if S_M >= 0 (S*_L >= 0 implies S_M >= 0)
-  const bool left = (SM >= 0.0);
-  const bool dbl = left ? !(SsL >= 0.0) : !(SsR <= 0.0);
-  HlldSide a;
-  a.rho = left ? L.rho : R.rho; a.u = left ? L.u : R.u; a.v = left ? L.v : R.v; a.w = left ? L.w : R.w;
-  a.by = left ? L.by : R.by; a.bz = left ? L.bz : R.bz; a.pT = left ? L.pT : R.pT; a.e = left ? L.e : R.e;
-  a.rhos = left ? L.rhos : R.rhos; a.vs = left ? L.vs : R.vs; a.ws = left ? L.ws : R.ws;
-  a.bys = left ? L.bys : R.bys; a.bzs = left ? L.bzs : R.bzs;
-  a.Su = left ? L.Su : R.Su; a.iSSm = left ? L.iSSm : R.iSSm;
-  const double S = left ? SL : SR;
-  const double vb = a.u * bx + a.v * a.by + a.w * a.bz;
-  const double vbs = SM * bx + a.vs * a.bys + a.ws * a.bzs;
-  const double es = (a.Su * a.e - a.pT * a.u + pTs * SM + bx * (vb - vbs)) * a.iSSm;  // M&K Eq. 48
-  F7 F = phys_flux(a, bx);
-  const double Usmt1 = a.rhos * a.vs, Usmt2 = a.rhos * a.ws;
-  // F*_a = F_a + S_a (U*_a - U_a)
-  F.m += S * (a.rhos - a.rho);
-  F.mn += S * (a.rhos * SM - a.rho * a.u);
-  F.mt1 += S * (Usmt1 - a.rho * a.v);
-  F.mt2 += S * (Usmt2 - a.rho * a.w);
-  F.e += S * (es - a.e);
-  F.by += S * (a.bys - a.by);
-  F.bz += S * (a.bzs - a.bz);
-  if (dbl) {
-    // double-star states (M&K Eq. 59-63)
-    const double Ss = left ? SsL : SsR;
-    double sgn = (bx > 0.0) ? 1.0 : ((bx < 0.0) ? -1.0 : 0.0);
-    double inv = rcp(rL + rR);
-    double vss = (rL * L.vs + rR * R.vs + (R.bys - L.bys) * sgn) * inv;
-    double wss = (rL * L.ws + rR * R.ws + (R.bzs - L.bzs) * sgn) * inv;
-    double byss = (rL * R.bys + rR * L.bys + rL * rR * (R.vs - L.vs) * sgn) * inv;
-    double bzss = (rL * R.bzs + rR * L.bzs + rL * rR * (R.ws - L.ws) * sgn) * inv;
-    double vbss = SM * bx + vss * byss + wss * bzss;
-    double r = left ? -rL : rR;
-    double ess = es + r * (vbs - vbss) * sgn;
-    // F**_a = F*_a + S*_a (U**_a - U*_a); rho** = rho*, u** = S_M
-    F.mt1 += Ss * (a.rhos * vss - Usmt1);
-    F.mt2 += Ss * (a.rhos * wss - Usmt2);
-    F.e += Ss * (ess - es);
-    F.by += Ss * (byss - a.bys);
-    F.bz += Ss * (bzss - a.bzs);
-    // mass and normal momentum: U** - U* = 0 exactly
+  // the state whose flux is the answer, and the total pressure it is under
+  double frho, fu, fv, fw, fby, fbz, fe, fpT, fvb, cb = 0.0, cby = 0.0, cbz = 0.0;
+  if (SL > 0.0 || SR < 0.0) {
+    const bool l = SL > 0.0;
+    frho = l ? L.rho : R.rho; fu = l ? L.u : R.u; fv = l ? L.v : R.v; fw = l ? L.w : R.w;
+    fby = l ? L.by : R.by; fbz = l ? L.bz : R.bz; fpT = l ? L.pT : R.pT;
+    fe = total_energy(gm1inv, frho, fu, fv, fw, l ? L.P : R.P, l ? L.hb2 : R.hb2);
+    fvb = fu * bx + fv * fby + fw * fbz;
+  } else {
+    // middle wave (M&K Eq. 38)
+    const double sduL = (SL - L.u) * L.rho;
+    const double sduR = (SR - R.u) * R.rho;
+    const double SM = (sduR * R.u - sduL * L.u - R.pT + L.pT) * rcp(sduR - sduL);
+    // side a bounds the face: left if S_M >= 0 (S*_L >= 0 implies S_M >= 0); b is the other one
+    const bool left = (SM >= 0.0);
+    const double a_rho = left ? L.rho : R.rho, a_u = left ? L.u : R.u, a_v = left ? L.v : R.v;
+    const double a_w = left ? L.w : R.w, a_P = left ? L.P : R.P, a_by = left ? L.by : R.by;
+    const double a_bz = left ? L.bz : R.bz, a_hb2 = left ? L.hb2 : R.hb2, a_pT = left ? L.pT : R.pT;
+    const double a_S = left ? SL : SR, a_sdu = left ? sduL : sduR;
+    const double dua = SM - a_u;
+    // total pressure of the fan from the jump across S_a (M&K Eq. 23; Eq. 41 is the same quantity)
+    const double pTs = a_pT + a_sdu * dua;
+    const Star A = hlld_star(a_S, SM, a_sdu, dua, a_v, a_w, a_by, a_bz, pTs, bx, bx2);
+    const double a_e = total_energy(gm1inv, a_rho, a_u, a_v, a_w, a_P, a_hb2);
+    const double vb = a_u * bx + a_v * a_by + a_w * a_bz;
+    const double vbs = SM * bx + A.vs * A.bys + A.ws * A.bzs;
+    const double es = ((a_S - a_u) * a_e - a_pT * a_u + pTs * SM + bx * (vb - vbs)) * A.iSSm;  // M&K Eq. 48
+    cb = A.degen ? -dua : 0.0;
+    cby = a_by; cbz = a_bz;
+    frho = A.rhos; fu = SM; fpT = pTs;
+    fv = A.vs; fw = A.ws; fby = A.bys; fbz = A.bzs; fe = es; fvb = vbs;
+    // double-star region: |S_M| < |B_x| / sqrt(rho*_a)   (S*_L < 0 <= S_M, or S_M < 0 < S*_R)
+    if (SM * SM * A.rhos < bx2) {
+      const double b_u = left ? R.u : L.u, b_v = left ? R.v : L.v, b_w = left ? R.w : L.w;
+      const double b_by = left ? R.by : L.by, b_bz = left ? R.bz : L.bz;
+      const double b_S = left ? SR : SL, b_sdu = left ? sduR : sduL;
+      const Star B = hlld_star(b_S, SM, b_sdu, SM - b_u, b_v, b_w, b_by, b_bz, pTs, bx, bx2);
+      // M&K Eq. 59-63, written for (a, b) with s' = sgn(B_x) for a = L and -sgn(B_x) for a = R
+      const double ra = sqrt_nz(A.rhos), rb = sqrt_nz(B.rhos);
+      const double sg = (bx > 0.0) ? 1.0 : ((bx < 0.0) ? -1.0 : 0.0);
+      const double sp = left ? sg : -sg;
+      const double inv = rcp(ra + rb);
+      const double rr = (ra * rb) * sp;
+      fv = (ra * A.vs + rb * B.vs + (B.bys - A.bys) * sp) * inv;
+      fw = (ra * A.ws + rb * B.ws + (B.bzs - A.bzs) * sp) * inv;
+      fby = (ra * B.bys + rb * A.bys + rr * (B.vs - A.vs)) * inv;
+      fbz = (ra * B.bzs + rb * A.bzs + rr * (B.ws - A.ws)) * inv;
+      fvb = SM * bx + fv * fby + fw * fbz;
+      fe = es - (ra * sp) * (vbs - fvb);
+    }
   }
+  F7 F = flux_of(frho, fu, fv, fw, fby, fbz, fe, fpT, fvb, bx, bx2);
+  F.by += cby * cb;   // degenerate star state of side a only (see the header); cb = 0 otherwise
+  F.bz += cbz * cb;
   // reading R6: a contact slower than 1e-13 of the fast speed is at rest -- the mass flux, whose
   // sign upwinds the CT terms (Eq. 16, G6), is then exactly zero ("otherwise" branch: average)
   if (fabs(F.m) <= 1e-13 * (L.rho + R.rho) * cfmax) F.m = 0.0;
@@ -202,40 +228,45 @@ __device__ __forceinline__ void eig_setup(Eig &e, double gamma, const W7 &W, dou
   double a, ia;
   sqrt_rsqrt(a2, a, ia);
   double ia2 = ia * ia;
-  double bp2 = W.by * W.by + W.bz * W.bz;
-  double s = gp + (bx * bx + bp2);
-  double disc = s * s - 4.0 * gp * bx * bx;
-  disc = disc < 0.0 ? 0.0 : disc;                 // reading R3
-  double cf2 = (s + sqrt_(disc)) * (0.5 * irho);  // Eq. 12
-  double ca2 = bx * bx * irho;
-  double cs2 = (cf2 > 0.0) ? a2 * ca2 * rcp(cf2) : 0.0;  // slow speed without cancellation (O9)
-  double cf = sqrt_(cf2), cs = sqrt_any(cs2);  // c_s^2 ~ B_n^2 can be denormal
-  if (bp2 == 0.0 && W.by == 0.0 && W.bz == 0.0) { e.betay = 1.0; e.betaz = 0.0; }
-  else {
-    // the numerical foot ahead of a switch-on shock carries transverse fields down to 1e-180 and
-    // below (Ryu & Jones 4d): rescale before squaring so that the seed instruction never sees a
-    // denormal (it flushes them to zero and the direction would come out as inf * 0)
-    double by = W.by, bz = W.bz;
-    if (fmax(fabs(by), fabs(bz)) < 0x1p-500) { by *= 0x1p600; bz *= 0x1p600; }
-    double ib = rsqrt_(by * by + bz * bz);
-    e.betay = by * ib; e.betaz = bz * ib;
+  double by = W.by, bz = W.bz;
+  double bx2 = bx * bx;
+  double s = gp + (bx2 + (by * by + bz * bz));
+  double disc = floor_tiny(s * s - 4.0 * gp * bx2);  // reading R3
+  double cf2 = (s + sqrt_nz(disc)) * (0.5 * irho);   // Eq. 12
+  // c_s = a c_a / c_f: no cancellation (O9), and no square of B_n, which can be ~1e-160 in the
+  // numerical foot of a switch-on shock (Ryu & Jones 4d, reading R12)
+  double icf = rsqrt_(cf2);
+  double cf = cf2 * icf;
+  double cs = (a * fabs(bx)) * (isr * icf);
+  double cs2 = cs * cs;
+  // direction of B_perp; (1, 0) when it vanishes (G16).  The same foot carries transverse fields
+  // down to 1e-180: rescale before squaring so that the seed instruction never sees a denormal
+  // (exponent test on the integer pipe)
+  int mag = max(hi32(by) & 0x7fffffff, hi32(bz) & 0x7fffffff);
+  if (mag < 0x20b00000) {  // max(|by|, |bz|) < 2^-500
+    by *= 0x1p600; bz *= 0x1p600;
+    if (by == 0.0 && bz == 0.0) by = 1.0;
   }
+  double ib = rsqrt_(by * by + bz * bz);
+  e.betay = by * ib; e.betaz = bz * ib;
   double dfs = cf2 - cs2;
-  if (dfs == 0.0) { e.alf = 1.0; e.als = 0.0; }
+  if (hi32(dfs) < 0x00100000) { e.alf = 1.0; e.als = 0.0; }  // c_f = c_s (G16)
   else {
     double idfs = rcp(dfs);
     double af2 = (a2 - cs2) * idfs;
     double as2 = (cf2 - a2) * idfs;
-    af2 = af2 < 0.0 ? 0.0 : (af2 > 1.0 ? 1.0 : af2);
-    as2 = as2 < 0.0 ? 0.0 : (as2 > 1.0 ? 1.0 : as2);
+    // clip to [0, 1] on the exponent bits: negative -> 0, >= 1 -> 1
+    af2 = hi32(af2) < 0 ? 0.0 : (hi32(af2) >= 0x3ff00000 ? 1.0 : af2);
+    as2 = hi32(as2) < 0 ? 0.0 : (hi32(as2) >= 0x3ff00000 ? 1.0 : as2);
     e.alf = sqrt_(af2); e.als = sqrt_(as2);
   }
-  double S = (bx >= 0.0) ? 1.0 : -1.0;
+  // S = sgn(B_n), +1 at 0 (O9): multiplication by S is a flip of the sign bit
+  const int sflip = (bx >= 0.0) ? 0 : (int)0x80000000;
   e.rho = rho; e.irho = irho; e.a2 = a2; e.ia2 = ia2; e.N = 0.5 * ia2;
   e.Cff = cf * e.alf; e.Css = cs * e.als;
-  e.Qf = e.Cff * S; e.Qs = e.Css * S;
+  e.Qf = xor_sign(e.Cff, sflip); e.Qs = xor_sign(e.Css, sflip);
   e.Af = a * e.alf * sr; e.As = a * e.als * sr;
-  e.Ssr = S * sr; e.Sisr = S * isr;
+  e.Ssr = xor_sign(sr, sflip); e.Sisr = xor_sign(isr, sflip);
 }
 
 // a = L . x   (x in the component order of W7).  Written with explicit rounding intrinsics so
@@ -288,15 +319,23 @@ __device__ __forceinline__ W7 eig_right(const Eig &e, const C7 &c) {
 // ---------------------------------------------------------------------------------------
 // PLMC, Eq. 23-28 (reading O8).  Out: Wlo = W_{R,i-1/2}, Whi = W_{L,i+1/2}.
 // ---------------------------------------------------------------------------------------
+// Sign tests and selections of the limiters run on the integer pipe (the sign of a double is
+// bit 63, its magnitude orders like the bit pattern); only the minima themselves are fp64 compares.
+__device__ __forceinline__ double min_pos(double a, double b) { return a < b ? a : b; }  // no NaN handling needed
+
 __device__ __forceinline__ double vl_slope(double dl, double dr) {  // Eq. 26 (G10)
-  return (dl * dr > 0.0) ? 2.0 * dl * dr * rcp(dl + dr) : 0.0;
+  // dl dr > 0 <=> the product is a positive normal number (a product that underflows gives a slope
+  // below 1e-300: zero for every purpose)
+  double pr = dl * dr;
+  return (hi32(pr) >= 0x00100000) ? 2.0 * pr * rcp(dl + dr) : 0.0;
 }
 
 __device__ __forceinline__ double plm_limit(double aL, double aR, double aC, double aVL) {  // Eq. 27
-  // min(2|aL|, 2|aR|, |aC|, |aVL|) with the sign of aC; where aL aR > 0, aC = (aL + aR)/2 has their
-  // sign and is non-zero, so the sign transfer is a bit operation
-  double m = fmin(2.0 * fmin(fabs(aL), fabs(aR)), fmin(fabs(aC), fabs(aVL)));
-  return (aL * aR > 0.0) ? copysign(m, aC) : 0.0;
+  // min(2|aL|, 2|aR|, |aC|, |aVL|) with the sign of aC where aL aR > 0, else 0.  If either of aL, aR
+  // is zero the minimum is zero by itself, so only "opposite signs" needs a test: the xor of the
+  // sign bits.  Where aL aR > 0, aC = (aL + aR)/2 has their sign: the sign transfer is a bit operation.
+  double m = min_pos(2.0 * min_pos(fabs(aL), fabs(aR)), min_pos(fabs(aC), fabs(aVL)));
+  return ((hi32(aL) ^ hi32(aR)) < 0) ? 0.0 : copysign(m, aC);
 }
 
 __device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, const W7 &Wp,

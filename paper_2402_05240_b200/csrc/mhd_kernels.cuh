@@ -217,7 +217,7 @@ __device__ __forceinline__ void pcm_face(double (*st)[MHD_PRED_T], const State8 
   double bn;
   W7 WL = to_W<A>(pm, bn);
   W7 WR = to_W<A>(pc, bn);
-  F7 f = hlld(g.gamma, g.gm1inv, WL, WR, pm.ir, pc.ir, __ldg(U.f[F_BX + A] + idx));
+  F7 f = hlld(g.gamma, g.gm1inv, WL, WR, __ldg(U.f[F_BX + A] + idx));
   store_flux<A>(F, idx, f);
 }
 
@@ -475,7 +475,7 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) 
   WL.rho = shfl_up1(hi.rho); WL.u = shfl_up1(hi.u); WL.v = shfl_up1(hi.v); WL.w = shfl_up1(hi.w);
   WL.P = shfl_up1(hi.P); WL.by = shfl_up1(hi.by); WL.bz = shfl_up1(hi.bz);
   if (active && lane >= 1) {
-    F7 f = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX] + idx));
+    F7 f = hlld(g.gamma, g.gm1inv, WL, lo, __ldg(Uh.f[F_BX] + idx));
     store_flux<0>(F, idx, f);
   }
 }
@@ -607,7 +607,7 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
     }
     reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
     if (f >= f0) {
-      F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, rcp(WL.rho), rcp(lo.rho), __ldg(Uh.f[F_BX + A] + idx));
+      F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, __ldg(Uh.f[F_BX + A] + idx));
       if (!UPDATE) {
         store_flux<A>(F, idx, fl);
       } else {

@@ -45,12 +45,27 @@ __device__ __forceinline__ double rsqrt_(double x) {
 __device__ __forceinline__ double sqrt_(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = __fma_rn(-(0.5 * x) * y, y, 0.5);
-  y = __fma_rn(y, e, y);
-  double s = x * y;
-  double r = __fma_rn(-s, s, x);  // residual x - s^2
-  s = __fma_rn(r, 0.5 * y, s);
-  return (x == 0.0) ? 0.0 : s;
+  double g = x * y, h = 0.5 * y;
+  double r = __fma_rn(-g, h, 0.5);
+  g = __fma_rn(g, r, g);
+  h = __fma_rn(h, r, h);
+  r = __fma_rn(-g, g, x);  // residual x - g^2
+  g = __fma_rn(r, h, g);
+  // zero test on the exponent bits (integer pipe; the seed instruction flushes denormals anyway)
+  return (__double2hiint(x) < 0x00100000) ? 0.0 : g;
+}
+
+// sqrt(x) for normal x > 0 only (no zero check): coupled iteration g -> sqrt(x), h -> 1/(2 sqrt(x))
+// from the hardware seed (one step, error 2^-43) and the correction g += (x - g^2) h.
+__device__ __forceinline__ double sqrt_nz(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double r = __fma_rn(-g, h, 0.5);
+  g = __fma_rn(g, r, g);
+  h = __fma_rn(h, r, h);
+  r = __fma_rn(-g, g, x);
+  return __fma_rn(r, h, g);
 }
 
 // sqrt(x) for x >= 0 of ANY magnitude, denormals included (the seed instruction flushes them to

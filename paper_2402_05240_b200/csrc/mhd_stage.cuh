@@ -69,7 +69,7 @@ __device__ __forceinline__ F7 stage_face(const Geo &g, const Prim &pm, const Pri
   double bn;
   W7 WL = to_W<A>(pm, bn);
   W7 WR = to_W<A>(pc, bn);
-  return hlld(g.gamma, g.gm1inv, WL, WR, pm.ir, pc.ir, bface);
+  return hlld(g.gamma, g.gm1inv, WL, WR, bface);
 }
 
 // hb = cells of the half state, [lo, hi] per axis; faces and edges are produced on [lo, hi+1].

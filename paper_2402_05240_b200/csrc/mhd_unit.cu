@@ -27,7 +27,7 @@ __global__ void k_unit_hlld(int n, double gamma, const double *WL, const double 
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
   W7 L = load_W(WL + 7 * t), R = load_W(WR + 7 * t);
-  F7 f = hlld(gamma, 1.0 / (gamma - 1.0), L, R, rcp(L.rho), rcp(R.rho), bx[t]);
+  F7 f = hlld(gamma, 1.0 / (gamma - 1.0), L, R, bx[t]);
   double *o = F + 7 * t;
   o[0] = f.m; o[1] = f.mn; o[2] = f.mt1; o[3] = f.mt2; o[4] = f.e; o[5] = f.by; o[6] = f.bz;
 }
