@@ -189,7 +189,7 @@ int launch_predictor_stage() {
   const int r = recon_radius(g.recon);
   Box hb;
   for (int a = 0; a < 3; a++) { hb.lo[a] = -1 - r; hb.hi[a] = g.n[a] + r; }
-  if (C.stage_ty == 12) return launch_stage_kernel<12>(hb);
+  if (C.stage_ty != 0) return launch_stage_kernel<MHD_STAGE_TY>(hb);
   Box pb;
   for (int a = 0; a < 3; a++) { pb.lo[a] = -2 - r; pb.hi[a] = g.n[a] + r + 1; }
   {
@@ -319,7 +319,7 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
   if (!make_geo(g, nx, ny, nz, gamma, recon)) return fail(MHD_ERR_ARG, "mhd_init: bad argument");
   {
     const int cols = MHD_STAGE_COLS * 32 * (int)sizeof(double);
-    CU(cudaFuncSetAttribute(k_predictor_stage<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols * 12));
+    CU(cudaFuncSetAttribute(k_predictor_stage<MHD_STAGE_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols * MHD_STAGE_TY));
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));

@@ -50,6 +50,9 @@ __device__ __forceinline__ double fast_speed_sq(double gamma, double irho, doubl
 // where the double-star state is needed, and no reciprocal of rho_L, rho_R is taken at all
 // (the larger fast speed is found by cross-multiplication).  ~200 fp64 instructions per solve.
 // ---------------------------------------------------------------------------------------
+#ifndef MHD_DBL_ALWAYS
+#define MHD_DBL_ALWAYS 0   // 1: form the double-star state on every face and select (one larger basic block)
+#endif
 __device__ __forceinline__ int hi32(double x) { return __double2hiint(x); }
 __device__ __forceinline__ double xor_sign(double x, int signbit) {
   return __hiloint2double(__double2hiint(x) ^ signbit, __double2loint(x));
@@ -139,15 +142,11 @@ __device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, co
   const double SR = (ul ? R.u : L.u) + cfmax;
 
   // the state whose flux is the answer, and the total pressure it is under
-  double frho, fu, fv, fw, fby, fbz, fe, fpT, fvb, cb = 0.0, cby = 0.0, cbz = 0.0;
-  if (SL > 0.0 || SR < 0.0) {
-    const bool l = SL > 0.0;
-    frho = l ? L.rho : R.rho; fu = l ? L.u : R.u; fv = l ? L.v : R.v; fw = l ? L.w : R.w;
-    fby = l ? L.by : R.by; fbz = l ? L.bz : R.bz; fpT = l ? L.pT : R.pT;
-    fe = total_energy(gm1inv, frho, fu, fv, fw, l ? L.P : R.P, l ? L.hb2 : R.hb2);
-    fvb = fu * bx + fv * fby + fw * fbz;
-  } else {
-    // middle wave (M&K Eq. 38)
+  double frho, fu, fv, fw, fby, fbz, fe, fpT, fvb, cb, cby, cbz;
+  const bool super = (SL > 0.0 || SR < 0.0);
+  {
+    // middle wave (M&K Eq. 38).  rho_R (S_R - u_R) > 0 > rho_L (S_L - u_L) always, so this block is
+    // well defined on supersonic faces too (its result is replaced below): no branch ahead of it
     const double sduL = (SL - L.u) * L.rho;
     const double sduR = (SR - R.u) * R.rho;
     const double SM = (sduR * R.u - sduL * L.u - R.pT + L.pT) * rcp(sduR - sduL);
@@ -170,7 +169,8 @@ __device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, co
     frho = A.rhos; fu = SM; fpT = pTs;
     fv = A.vs; fw = A.ws; fby = A.bys; fbz = A.bzs; fe = es; fvb = vbs;
     // double-star region: |S_M| < |B_x| / sqrt(rho*_a)   (S*_L < 0 <= S_M, or S_M < 0 < S*_R)
-    if (SM * SM * A.rhos < bx2) {
+    const bool dbl = SM * SM * A.rhos < bx2;
+    if (MHD_DBL_ALWAYS || dbl) {
       const double b_u = left ? R.u : L.u, b_v = left ? R.v : L.v, b_w = left ? R.w : L.w;
       const double b_by = left ? R.by : L.by, b_bz = left ? R.bz : L.bz;
       const double b_S = left ? SR : SL, b_sdu = left ? sduR : sduL;
@@ -181,13 +181,22 @@ __device__ __forceinline__ F7 hlld(double gamma, double gm1inv, const W7 &WL, co
       const double sp = left ? sg : -sg;
       const double inv = rcp(ra + rb);
       const double rr = (ra * rb) * sp;
-      fv = (ra * A.vs + rb * B.vs + (B.bys - A.bys) * sp) * inv;
-      fw = (ra * A.ws + rb * B.ws + (B.bzs - A.bzs) * sp) * inv;
-      fby = (ra * B.bys + rb * A.bys + rr * (B.vs - A.vs)) * inv;
-      fbz = (ra * B.bzs + rb * A.bzs + rr * (B.ws - A.ws)) * inv;
-      fvb = SM * bx + fv * fby + fw * fbz;
-      fe = es - (ra * sp) * (vbs - fvb);
+      const double vss = (ra * A.vs + rb * B.vs + (B.bys - A.bys) * sp) * inv;
+      const double wss = (ra * A.ws + rb * B.ws + (B.bzs - A.bzs) * sp) * inv;
+      const double byss = (ra * B.bys + rb * A.bys + rr * (B.vs - A.vs)) * inv;
+      const double bzss = (ra * B.bzs + rb * A.bzs + rr * (B.ws - A.ws)) * inv;
+      const double vbss = SM * bx + vss * byss + wss * bzss;
+      const double ess = es - (ra * sp) * (vbs - vbss);
+      if (dbl) { fv = vss; fw = wss; fby = byss; fbz = bzss; fvb = vbss; fe = ess; }
     }
+  }
+  if (super) {   // S_L > 0: F_L; S_R < 0: F_R (rare; after the main block so that it stays in one piece)
+    const bool l = SL > 0.0;
+    frho = l ? L.rho : R.rho; fu = l ? L.u : R.u; fv = l ? L.v : R.v; fw = l ? L.w : R.w;
+    fby = l ? L.by : R.by; fbz = l ? L.bz : R.bz; fpT = l ? L.pT : R.pT;
+    fe = total_energy(gm1inv, frho, fu, fv, fw, l ? L.P : R.P, l ? L.hb2 : R.hb2);
+    fvb = fu * bx + fv * fby + fw * fbz;
+    cb = 0.0;
   }
   F7 F = flux_of(frho, fu, fv, fw, fby, fbz, fe, fpT, fvb, bx, bx2);
   F.by += cby * cb;   // degenerate star state of side a only (see the header); cb = 0 otherwise
@@ -338,30 +347,26 @@ __device__ __forceinline__ double plm_limit(double aL, double aR, double aC, dou
   return ((hi32(aL) ^ hi32(aR)) < 0) ? 0.0 : copysign(m, aC);
 }
 
-__device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, const W7 &Wp,
-                                     double bx0, W7 &Wlo, W7 &Whi) {
+// from the one-sided differences dL = W_i - W_{i-1} (Eq. 23), dR = W_{i+1} - W_i (Eq. 24): a marching
+// sweep carries dR over as the next cell's dL
+__device__ __forceinline__ void plmc_d(double gamma, const W7 &W0, const W7 &dL, const W7 &dR, double bx0,
+                                       W7 &Wlo, W7 &Whi) {
   Eig e;
   eig_setup(e, gamma, W0, bx0);
-  W7 dL, dR, dV;
-#define MHD_D4(f)                                   \
-  dL.f = W0.f - Wm.f; dR.f = Wp.f - W0.f;           \
-  dV.f = vl_slope(dL.f, dR.f);
-  MHD_D4(rho) MHD_D4(u) MHD_D4(v) MHD_D4(w) MHD_D4(P) MHD_D4(by) MHD_D4(bz)
-#undef MHD_D4
+  W7 dV;
+  dV.rho = vl_slope(dL.rho, dR.rho); dV.u = vl_slope(dL.u, dR.u); dV.v = vl_slope(dL.v, dR.v);
+  dV.w = vl_slope(dL.w, dR.w); dV.P = vl_slope(dL.P, dR.P); dV.by = vl_slope(dL.by, dR.by);
+  dV.bz = vl_slope(dL.bz, dR.bz);
   // L is linear and dC = (dL + dR)/2, so the centred amplitudes are the mean of the one-sided ones
   C7 aL = eig_left(e, dL), aR = eig_left(e, dR), aV = eig_left(e, dV);
-  C7 aC;
-  aC.c0 = 0.5 * (aL.c0 + aR.c0); aC.c1 = 0.5 * (aL.c1 + aR.c1); aC.c2 = 0.5 * (aL.c2 + aR.c2);
-  aC.c3 = 0.5 * (aL.c3 + aR.c3); aC.c4 = 0.5 * (aL.c4 + aR.c4); aC.c5 = 0.5 * (aL.c5 + aR.c5);
-  aC.c6 = 0.5 * (aL.c6 + aR.c6);
   C7 am;
-  am.c0 = plm_limit(aL.c0, aR.c0, aC.c0, aV.c0);
-  am.c1 = plm_limit(aL.c1, aR.c1, aC.c1, aV.c1);
-  am.c2 = plm_limit(aL.c2, aR.c2, aC.c2, aV.c2);
-  am.c3 = plm_limit(aL.c3, aR.c3, aC.c3, aV.c3);
-  am.c4 = plm_limit(aL.c4, aR.c4, aC.c4, aV.c4);
-  am.c5 = plm_limit(aL.c5, aR.c5, aC.c5, aV.c5);
-  am.c6 = plm_limit(aL.c6, aR.c6, aC.c6, aV.c6);
+  am.c0 = plm_limit(aL.c0, aR.c0, 0.5 * (aL.c0 + aR.c0), aV.c0);
+  am.c1 = plm_limit(aL.c1, aR.c1, 0.5 * (aL.c1 + aR.c1), aV.c1);
+  am.c2 = plm_limit(aL.c2, aR.c2, 0.5 * (aL.c2 + aR.c2), aV.c2);
+  am.c3 = plm_limit(aL.c3, aR.c3, 0.5 * (aL.c3 + aR.c3), aV.c3);
+  am.c4 = plm_limit(aL.c4, aR.c4, 0.5 * (aL.c4 + aR.c4), aV.c4);
+  am.c5 = plm_limit(aL.c5, aR.c5, 0.5 * (aL.c5 + aR.c5), aV.c5);
+  am.c6 = plm_limit(aL.c6, aR.c6, 0.5 * (aL.c6 + aR.c6), aV.c6);
   W7 dW = eig_right(e, am);
 #define MHD_O(f) Whi.f = W0.f + dW.f / 2.0; Wlo.f = W0.f - dW.f / 2.0;
   MHD_O(rho) MHD_O(u) MHD_O(v) MHD_O(w) MHD_O(P) MHD_O(by) MHD_O(bz)
@@ -369,15 +374,31 @@ __device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, c
 }
 
 // PLMP (limiting in the primitive variables = Eq. 23-28 without the projections)
-__device__ __forceinline__ void plmp(const W7 &Wm, const W7 &W0, const W7 &Wp, W7 &Wlo, W7 &Whi) {
+__device__ __forceinline__ void plmp_d(const W7 &W0, const W7 &dL, const W7 &dR, W7 &Wlo, W7 &Whi) {
 #define MHD_P1(f)                                                                        \
   {                                                                                      \
-    double dl = W0.f - Wm.f, dr = Wp.f - W0.f;                                           \
+    double dl = dL.f, dr = dR.f;                                                         \
     double dm = plm_limit(dl, dr, 0.5 * (dl + dr), vl_slope(dl, dr));                    \
     Whi.f = W0.f + 0.5 * dm; Wlo.f = W0.f - 0.5 * dm;                                    \
   }
   MHD_P1(rho) MHD_P1(u) MHD_P1(v) MHD_P1(w) MHD_P1(P) MHD_P1(by) MHD_P1(bz)
 #undef MHD_P1
+}
+
+__device__ __forceinline__ W7 w7_diff(const W7 &a, const W7 &b) {
+  W7 d;
+  d.rho = a.rho - b.rho; d.u = a.u - b.u; d.v = a.v - b.v; d.w = a.w - b.w; d.P = a.P - b.P;
+  d.by = a.by - b.by; d.bz = a.bz - b.bz;
+  return d;
+}
+
+__device__ __forceinline__ void plmc(double gamma, const W7 &Wm, const W7 &W0, const W7 &Wp,
+                                     double bx0, W7 &Wlo, W7 &Whi) {
+  plmc_d(gamma, W0, w7_diff(W0, Wm), w7_diff(Wp, W0), bx0, Wlo, Whi);
+}
+
+__device__ __forceinline__ void plmp(const W7 &Wm, const W7 &W0, const W7 &Wp, W7 &Wlo, W7 &Whi) {
+  plmp_d(W0, w7_diff(W0, Wm), w7_diff(Wp, W0), Wlo, Whi);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -473,8 +494,13 @@ __device__ __forceinline__ void ppmp(const W7 &Wm2, const W7 &Wm1, const W7 &W0,
 // faces; Er00, Er10, Er01, Er11 = reference field of cells (ia,ib), (ia-1,ib), (ia,ib-1),
 // (ia-1,ib-1).  All Delta factors of Eq. 15 and 17 cancel.
 // ---------------------------------------------------------------------------------------
+// Eq. 16 (G6): upwind by the sign of the interface mass flux, average where it is zero.  Every mass
+// flux comes out of hlld(), which returns either +0.0 (reading R6) or a normal number, so the sign
+// and the zero are read off the upper word on the integer pipe.
 __device__ __forceinline__ double upwind(double M, double from_lower, double from_upper) {
-  return (M > 0.0) ? from_lower : ((M < 0.0) ? from_upper : 0.5 * (from_lower + from_upper));
+  const int h = hi32(M);
+  const double avg = 0.5 * (from_lower + from_upper);
+  return (h >= 0x00100000) ? from_lower : ((h < 0 && h != (int)0x80000000) ? from_upper : avg);
 }
 
 __device__ __forceinline__ double ct_edge(double Ea0, double Ea1, double Eb0, double Eb1, double Ma0,

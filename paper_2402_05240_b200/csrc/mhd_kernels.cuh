@@ -241,6 +241,9 @@ __device__ __forceinline__ void pcm_face(double (*st)[MHD_PRED_T], const State8 
 #ifndef MHD_MINB_FM
 #define MHD_MINB_FM 4
 #endif
+#ifndef MHD_MINB_FMZ
+#define MHD_MINB_FMZ 3
+#endif
 #ifndef MHD_MINB_FM_PPM
 #define MHD_MINB_FM_PPM 3
 #endif
@@ -492,7 +495,7 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) 
 // do, for the CT kernel), and the full update that follows only has the face field left to do.
 // A chunk then also solves face f1+1 (its last cell needs it; 1/J more Riemann solves).
 template <int A, int RC, bool UPDATE>
-__global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
+__global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM : (UPDATE ? MHD_MINB_FMZ : MHD_MINB_FM)) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
                                                                   State8 U, const Scalars *sc) {
   static_assert(!UPDATE || A == 2, "the fused hydro update rides on the z sweep");
   constexpr int R = recon_radius(RC);
@@ -518,8 +521,11 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
   // 5-cell (PPM) sweeps: the window lives in this thread's column of shared memory (ring of 5 slots)
   // between iterations, so that its 40 doubles do not sit in registers across the projections
   // (dynamic shared memory, MHD_WSM_BYTES per block: with the update operands of the z sweep the
-  // total exceeds the 48 KB static limit)
+  // total exceeds the 48 KB static limit).
+  // 3-cell (PLM) sweeps carry cell f and its lower one-sided difference dL = W_f - W_{f-1} (Eq. 23);
+  // dR = W_{f+1} - W_f (Eq. 24) becomes the next cell's dL.
   constexpr bool WSM = (R == 2);
+  constexpr bool PLM = (R == 1);
   extern __shared__ double wsm_[];
   auto wput = [&](int slot, const W7 &W, double bn) {
     double *q = wsm_ + slot * 8 * 128 + threadIdx.x;
@@ -529,19 +535,27 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
     const double *q = wsm_ + slot * 8 * 128 + threadIdx.x;
     W.rho = q[0]; W.u = q[128]; W.v = q[256]; W.w = q[384]; W.P = q[512]; W.by = q[640]; W.bz = q[768]; bn = q[896];
   };
-  // window centred on cell f0-2 (slot 0 is never used): the loop below first shifts it
+  W7 W0c, dLc;
+  double bn0c = 0.0;
+  if constexpr (PLM) {
+    double bnm;
+    const W7 Wm = to_W<A>(load_prim_half(Uh, g, idx - 2 * sA), bnm);
+    W0c = to_W<A>(load_prim_half(Uh, g, idx - sA), bn0c);
+    dLc = w7_diff(W0c, Wm);
+  } else {
+    // window centred on cell f0-2 (slot 0 is never used): the loop below first shifts it
 #pragma unroll
-  for (int s = 1; s < 2 * R + 1; s++) {
-    Prim p = load_prim_half(Uh, g, idx + (long long)(s - R - 2) * sA);
-    win[s] = to_W<A>(p, bnc[s]);
-    if (WSM) wput(s, win[s], bnc[s]);   // ring position of window slot s at "time" 0
+    for (int s = 1; s < 2 * R + 1; s++) {
+      Prim p = load_prim_half(Uh, g, idx + (long long)(s - R - 2) * sA);
+      win[s] = to_W<A>(p, bnc[s]);
+      if (WSM) wput(s, win[s], bnc[s]);   // ring position of window slot s at "time" 0
+    }
+    if constexpr (R > 0) { win[0] = win[1]; bnc[0] = bnc[1]; }
+    if (WSM) wput(0, win[0], bnc[0]);
   }
-  if constexpr (R > 0) { win[0] = win[1]; bnc[0] = bnc[1]; }
-  if (WSM) wput(0, win[0], bnc[0]);
   int ring = 0;  // ring slot that holds window slot 0
   W7 WL, lo, hi;
-  if constexpr (R > 0) WL = win[1];
-  else WL.rho = WL.u = WL.v = WL.w = WL.P = WL.by = WL.bz = 0.0;  // (replaced before its first use)
+  WL.rho = WL.P = 1.0; WL.u = WL.v = WL.w = WL.by = WL.bz = 0.0;  // (replaced before its first use)
   F7 fprev;
   fprev.m = fprev.mn = fprev.mt1 = fprev.mt2 = fprev.e = fprev.by = fprev.bz = 0.0;
   // staging column of this thread: slots 0..4 = U (rho, mx, my, mz, E) of the cell to update,
@@ -574,38 +588,38 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM) 
   // cell is then reconstructed by the same instruction sequence, so mirror-image cells give
   // mirror-image states bit for bit.
   for (int f = f0 - 1; f <= fend; f++, idx += sA) {
-    if (!WSM) {
-#pragma unroll
-      for (int s = 0; s < 2 * R; s++) { win[s] = win[s + 1]; bnc[s] = bnc[s + 1]; }
-    }
-    {
+    if constexpr (PLM) {
+      cp_async_wait_but_last();  // the prefetch of cell f+1 (the newer group is the update's)
+      const int b = f & 1;
       Prim p;
-      if (PREF) {
-        cp_async_wait_but_last();  // the prefetch of this iteration's cell (the newer group is the update's)
-        const int b = f & 1;
-        p.rho = pre[b][0][tid]; p.ir = 0.0;
-        p.v[0] = pre[b][1][tid]; p.v[1] = pre[b][2][tid]; p.v[2] = pre[b][3][tid];
-        p.P = pre[b][4][tid];
-        p.B[0] = 0.5 * (pre[b][5][tid] + pre[b][6][tid]);
-        p.B[1] = 0.5 * (pre[b][7][tid] + pre[b][8][tid]);
-        p.B[2] = 0.5 * (pre[b][9][tid] + pre[b][10][tid]);
-        if (f < fend) prefetch(b ^ 1, idx + (long long)(R + 1) * sA);
-      } else {
-        p = load_prim_half(Uh, g, idx + (long long)R * sA);
-      }
-      win[2 * R] = to_W<A>(p, bnc[2 * R]);
+      p.rho = pre[b][0][tid]; p.ir = 0.0;
+      p.v[0] = pre[b][1][tid]; p.v[1] = pre[b][2][tid]; p.v[2] = pre[b][3][tid];
+      p.P = pre[b][4][tid];
+      p.B[0] = 0.5 * (pre[b][5][tid] + pre[b][6][tid]);
+      p.B[1] = 0.5 * (pre[b][7][tid] + pre[b][8][tid]);
+      p.B[2] = 0.5 * (pre[b][9][tid] + pre[b][10][tid]);
+      if (f < fend) prefetch(b ^ 1, idx + (long long)(R + 1) * sA);
       cp_async_commit();
-    }
-    if (WSM) {  // the oldest ring slot takes the new cell; the window is re-read slot by slot
-      wput(ring, win[2 * R], bnc[2 * R]);
-      ring = (ring + 1 == 5) ? 0 : ring + 1;
+      double bnp;
+      const W7 Wp = to_W<A>(p, bnp);
+      const W7 dR = w7_diff(Wp, W0c);
+      if (RC == 1) plmc_d(g.gamma, W0c, dLc, dR, bn0c, lo, hi);   // Eq. 23-28
+      else plmp_d(W0c, dLc, dR, lo, hi);
+      dLc = dR; W0c = Wp; bn0c = bnp;
+    } else {
+      win[2 * R] = to_W<A>(load_prim_half(Uh, g, idx + (long long)R * sA), bnc[2 * R]);
+      cp_async_commit();
+      if (WSM) {  // the oldest ring slot takes the new cell; the window is re-read slot by slot
+        wput(ring, win[2 * R], bnc[2 * R]);
+        ring = (ring + 1 == 5) ? 0 : ring + 1;
 #pragma unroll
-      for (int s = 0; s < 2 * R; s++) {
-        int slot = ring + s; slot = (slot >= 5) ? slot - 5 : slot;
-        wget(slot, win[s], bnc[s]);
+        for (int s = 0; s < 2 * R; s++) {
+          int slot = ring + s; slot = (slot >= 5) ? slot - 5 : slot;
+          wget(slot, win[s], bnc[s]);
+        }
       }
+      reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
     }
-    reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
     if (f >= f0) {
       F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, __ldg(Uh.f[F_BX + A] + idx));
       if (!UPDATE) {
