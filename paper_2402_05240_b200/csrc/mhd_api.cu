@@ -8,6 +8,7 @@
 #include "../../include/mhd.h"
 #include "mhd_kernels.cuh"
 #include "mhd_stage.cuh"
+#include "mhd_ctupdate.cuh"
 
 using namespace mhd;
 
@@ -38,6 +39,7 @@ struct Context {
   long long graph_launches = 0;
   int num_sms = 148;
   int stage_ty = MHD_STAGE_TY;  // rows per block of the fused predictor stage (0 = three kernels)
+  bool ct_fused = false;        // corrector CT + face update + CFL as one kernel (slower so far: per-plane barrier)
   int parity = 0;  // flips with every step (which set of face arrays holds B^n)
   // per-launch event timing (mhd_step_profile)
   int prof_n = -1;  // -1 = off, else number of launches recorded so far
@@ -108,11 +110,16 @@ void extents(int f, const Geo &g, int &ex, int &ey, int &ez) {
 
 int fill_ghosts(State8 &U) {
   const Geo &g = C.g;
-  const int B = 256;
-  const long long L0 = g.n[0] + 2 * g.ng, L1 = g.n[1] + 2 * g.ng;
-  long long t0 = L0 * L1 * 2 * g.ng, t1 = L0 * 2 * g.ng * g.n[2], t2 = 2LL * g.ng * g.n[1] * g.n[2];
-  long long tmax = t0 > t1 ? (t0 > t2 ? t0 : t2) : (t1 > t2 ? t1 : t2);
-  k_fill_ghosts<<<dim3(grid1(tmax, B).x, 3, NFIELD), B, 0, C.stream>>>(U, g);
+  const int L0 = g.n[0] + 2 * g.ng, L1 = g.n[1] + 2 * g.ng;
+  int B = round_up(L0, 32);                  // one thread per x index of a row (grid rows are short)
+  if (B > 1024) B = 1024;
+  if (B < 64) B = 64;
+  const int per = B / (2 * g.ng);            // grid rows per block in the x-column part
+  const long long rows = (long long)L1 * 2 * g.ng + 2LL * g.ng * g.n[2] + ((long long)g.n[1] * g.n[2] + per - 1) / per;
+  // grid.y <= 65535 holds far beyond what fits in 180 GB (640^3: 15 k rows; 1024^3: 25 k)
+  const long long brows = (rows + MHD_GHOST_RPB - 1) / MHD_GHOST_RPB;
+  if (brows > 65535) return fail(MHD_ERR_ARG, "grid too large for the ghost-fill launch");
+  k_fill_ghosts<<<dim3((L0 + B - 1) / B, (unsigned)brows, NFIELD), B, 0, C.stream>>>(U, g);
   LAUNCH_CHECK("k_fill_ghosts");
   return MHD_OK;
 }
@@ -228,22 +235,40 @@ int step_kernels() {
     default: rc = launch_corrector_fluxes<4>(); break;
   }
   if (rc) return rc;
-  // Step 8 (G12): CT with the corrector fluxes and the half-step reference state, indices [0, n]
-  // Step 9: full update of cells [0, n-1] and faces 0..n
+  // Step 8 (G12): CT with the corrector fluxes and the half-step reference state, indices [0, n];
+  // Step 9: faces 0..n of B^{n+1} (the hydro variables were updated by the z sweep); CFL rate of U^{n+1}.
+  // One kernel (mhd_ctupdate.cuh); MHD_CT_FUSED=0 at mhd_init selects the two separate kernels.
+  // B^{n+1} goes to a second set of face arrays which then become the state's (pointer swap): a thread
+  // reads B^n on faces owned by other threads.
   {
-    Box ab, eb;
-    for (int a = 0; a < 3; a++) { ab.lo[a] = 0; ab.hi[a] = g.n[a] - 1; eb.lo[a] = 0; eb.hi[a] = g.n[a]; }
-    long long plane = (long long)(g.n[0] + 1) * (g.n[1] + 1);
-    dim3 grid(grid1(plane, 256).x, g.n[2] + 1);
-    k_ct<<<grid, 256, 0, C.stream>>>(C.F, C.Er, C.E, g, eb);
-    LAUNCH_CHECK("k_ct(corrector)");
-    dim3 gridu(grid1(plane, 256).x, g.n[2] + 1);
-    // hydro fields in place; B^{n+1} goes to a second set of face arrays which then become the
-    // state's (pointer swap): a thread reads B^n on its upper faces, owned by other threads
     State8 out = C.U;
     for (int a = 0; a < 3; a++) out.f[F_BX + a] = C.Bnext.f[a];
-    k_update<false><<<gridu, 256, 0, C.stream>>>(C.U, out, C.F, C.E, C.Er, g, ab, C.sc, 1.0);
-    LAUNCH_CHECK("k_update(B)+cfl");
+    if (C.ct_fused) {
+      constexpr int TY = MHD_CTU_TY;
+      const int ntx = (g.n[0] + 1 + 30) / 31, nty = (g.n[1] + 1 + TY - 2) / (TY - 1);
+      const long long tiles = (long long)ntx * nty;
+      const long long slots = (long long)C.num_sms * MHD_MINB_CTU;
+      // z is cut into chunks so that the tiles fill the SMs in whole waves; every chunk pays one extra plane
+      int best = 1;
+      long long best_cost = -1;
+      const int nz = g.n[2];
+      for (int c = 1; c <= nz && c <= 64; c++) {
+        long long cost = ((tiles * c + slots - 1) / slots) * ((nz + c - 1) / c + 1);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = c; }
+      }
+      const int lz = (nz + best - 1) / best;
+      k_ct_update<TY><<<dim3((unsigned)tiles, (nz + lz - 1) / lz), 32 * TY, 0, C.stream>>>(C.U, C.Bnext, C.F, C.Er, g, C.sc, ntx, lz);
+      LAUNCH_CHECK("k_ct_update+cfl");
+    } else {
+      Box ab, eb;
+      for (int a = 0; a < 3; a++) { ab.lo[a] = 0; ab.hi[a] = g.n[a] - 1; eb.lo[a] = 0; eb.hi[a] = g.n[a]; }
+      long long plane = (long long)(g.n[0] + 1) * (g.n[1] + 1);
+      dim3 grid(grid1(plane, 256).x, g.n[2] + 1);
+      k_ct<<<grid, 256, 0, C.stream>>>(C.F, C.Er, C.E, g, eb);
+      LAUNCH_CHECK("k_ct(corrector)");
+      k_update<false><<<grid, 256, 0, C.stream>>>(C.U, out, C.F, C.E, C.Er, g, ab, C.sc, 1.0);
+      LAUNCH_CHECK("k_update(B)+cfl");
+    }
     for (int a = 0; a < 3; a++) { C.Bnext.f[a] = C.U.f[F_BX + a]; C.U.f[F_BX + a] = out.f[F_BX + a]; }
     C.parity ^= 1;
     C.rate_valid = true;
@@ -326,6 +351,8 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
     C.num_sms = sms > 0 ? sms : 148;
     const char *e = getenv("MHD_STAGE_TY");
     if (e) C.stage_ty = atoi(e);
+    e = getenv("MHD_CT_FUSED");
+    if (e) C.ct_fused = atoi(e) != 0;
   }
   size_t need = total_bytes(g);
   if (ws) {

@@ -19,9 +19,11 @@ namespace mhd {
 // (src_x(i), src_y(j), src_z(k)), where src_a is the per-axis boundary map; this kernel applies the
 // composed map directly.  Periodic: src = i mod n (so the upper boundary face of the normal field
 // copies face 0).  Outflow: nearest active cell, or nearest active face 0..n for the normal field.
-// blockIdx.z = field; blockIdx.y = region: 0 = the z ghost slabs over all (i, j), 1 = the y ghost
-// slabs over all i and active k, 2 = the x ghost columns over active (j, k) -- disjoint, together
-// every index with at least one ghost coordinate.
+// blockIdx.z = field; blockIdx.y = a row of the ghost region, decoded once per block (no per-thread
+// divisions): rows [0, R0) = (j, z slot) of the z ghost slabs over all (i, j); [R0, R0 + R1) = (y slot,
+// k) of the y ghost slabs over all i and active k -- one thread per i along the row, coalesced; the
+// remaining block rows cover the x ghost columns over active (j, k), 2 ng values per grid row and
+// blockDim.x / (2 ng) grid rows per block.  Disjoint, together every index with a ghost coordinate.
 // ---------------------------------------------------------------------------------------
 __device__ __forceinline__ int ghost_src(int i, int n, int bc, bool normalB) {
   if (bc == MHD_BC_PERIODIC) { int s = i % n; return s < 0 ? s + n : s; }
@@ -33,28 +35,50 @@ __device__ __forceinline__ int ghost_slot(int slot, int ng, int n) {  // slot 0.
   return slot < ng ? slot - ng : n + (slot - ng);
 }
 
-__global__ void __launch_bounds__(256) k_fill_ghosts(State8 U, Geo g) {
-  const int f = blockIdx.z, region = blockIdx.y;
+#define MHD_GHOST_RPB 8   // rows per block (blocks of one short row each are bound by the block launch rate)
+
+__global__ void __launch_bounds__(1024) k_fill_ghosts(State8 U, Geo g) {
+  const int f = blockIdx.z;
   const int ng = g.ng, n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
   const int L0 = n0 + 2 * ng, L1 = n1 + 2 * ng;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  int i, j, k;
-  if (region == 0) {
-    if (t >= (long long)L0 * L1 * 2 * ng) return;
-    i = (int)(t % L0) - ng; j = (int)((t / L0) % L1) - ng; k = ghost_slot((int)(t / ((long long)L0 * L1)), ng, n2);
-  } else if (region == 1) {
-    if (t >= (long long)L0 * 2 * ng * n2) return;
-    i = (int)(t % L0) - ng; j = ghost_slot((int)((t / L0) % (2 * ng)), ng, n1); k = (int)(t / ((long long)L0 * 2 * ng));
-  } else {
-    if (t >= 2LL * ng * n1 * n2) return;
-    i = ghost_slot((int)(t % (2 * ng)), ng, n0); j = (int)((t / (2 * ng)) % n1); k = (int)(t / (2LL * ng * n1));
-  }
-  const int si = ghost_src(i, n0, g.bc[0], f == F_BX);
-  const int sj = ghost_src(j, n1, g.bc[1], f == F_BY);
-  const int sk = ghost_src(k, n2, g.bc[2], f == F_BZ);
-  if (si == i && sj == j && sk == k) return;  // an active face of the normal field on an outflow side
+  const int R0 = L1 * 2 * ng, R1 = 2 * ng * n2;
+  const int per = blockDim.x / (2 * ng);                      // grid rows per block row in the x-column part
+  const long long nrow2 = (long long)n1 * n2;
+  const int R2 = (int)((nrow2 + per - 1) / per);
   double *p = U.f[f];
-  p[cell_index(g, i, j, k)] = p[cell_index(g, si, sj, sk)];
+  double v[MHD_GHOST_RPB];
+  long long dst[MHD_GHOST_RPB];
+#pragma unroll
+  for (int u = 0; u < MHD_GHOST_RPB; u++) {
+    int r = blockIdx.y * MHD_GHOST_RPB + u;
+    dst[u] = -1;
+    if (r >= R0 + R1 + R2) continue;
+    int i, j, k;
+    if (r < R0 + R1) {
+      i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+      if (i >= L0) continue;
+      i -= ng;
+      if (r < R0) { j = r % L1 - ng; k = ghost_slot(r / L1, ng, n2); }
+      else { r -= R0; j = ghost_slot(r % (2 * ng), ng, n1); k = r / (2 * ng); }
+    } else {
+      if (blockIdx.x != 0) continue;
+      const int q = (int)threadIdx.x / (2 * ng);
+      if (q >= per) continue;
+      const long long row = (long long)(r - R0 - R1) * per + q;   // (j, k) = row % n1, row / n1
+      if (row >= nrow2) continue;
+      i = ghost_slot((int)threadIdx.x - q * 2 * ng, ng, n0);
+      j = (int)(row % n1); k = (int)(row / n1);
+    }
+    const int si = ghost_src(i, n0, g.bc[0], f == F_BX);
+    const int sj = ghost_src(j, n1, g.bc[1], f == F_BY);
+    const int sk = ghost_src(k, n2, g.bc[2], f == F_BZ);
+    if (si == i && sj == j && sk == k) continue;  // an active face of the normal field on an outflow side
+    dst[u] = cell_index(g, i, j, k);
+    v[u] = p[cell_index(g, si, sj, sk)];
+  }
+#pragma unroll
+  for (int u = 0; u < MHD_GHOST_RPB; u++)
+    if (dst[u] >= 0) p[dst[u]] = v[u];
 }
 
 // ---------------------------------------------------------------------------------------
@@ -446,6 +470,12 @@ __device__ __forceinline__ void reconstruct(double gamma, const W7 *win, double 
 // Riemann problem on their lower face.  No shared memory, no block barrier; consecutive warps
 // overlap by one cell (1/31 of the reconstructions are done twice).
 __device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+// B + c (hi - lo) with one rounding per operation, identical wherever it is inlined
+__device__ __forceinline__ double fma_diff(double B, double c, double hi, double lo) {
+  return __fma_rn(c, __dadd_rn(hi, -lo), B);
+}
 
 template <int RC>
 __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) k_flux_x(State8 Uh, Flux21 F, Geo g, Box fb, int nwx) {
@@ -598,7 +628,11 @@ __global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM :
       p.B[0] = 0.5 * (pre[b][5][tid] + pre[b][6][tid]);
       p.B[1] = 0.5 * (pre[b][7][tid] + pre[b][8][tid]);
       p.B[2] = 0.5 * (pre[b][9][tid] + pre[b][10][tid]);
+#ifdef MHD_EXP_NOLOAD
+      if (f < fend) prefetch(b ^ 1, idx - (long long)(f - f0) * sA);
+#else
       if (f < fend) prefetch(b ^ 1, idx + (long long)(R + 1) * sA);
+#endif
       cp_async_commit();
       double bnp;
       const W7 Wp = to_W<A>(p, bnp);
@@ -623,6 +657,9 @@ __global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM :
     if (f >= f0) {
       F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, __ldg(Uh.f[F_BX + A] + idx));
       if (!UPDATE) {
+#ifdef MHD_EXP_NOSTORE
+        if (fl.m == 12345.678)
+#endif
         store_flux<A>(F, idx, fl);
       } else {
         if (f <= f1) { F.f[A][0][idx] = fl.m; F.f[A][5][idx] = fl.by; F.f[A][6][idx] = fl.bz; }

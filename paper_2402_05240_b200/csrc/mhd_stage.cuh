@@ -24,13 +24,6 @@ namespace mhd {
 #define MHD_STAGE_TY 12
 #endif
 
-__device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
-
-// B + c (hi - lo) with one rounding per operation, identical wherever it is inlined
-__device__ __forceinline__ double fma_diff(double B, double c, double hi, double lo) {
-  return __fma_rn(c, __dadd_rn(hi, -lo), B);
-}
-
 // Split-phase block barrier (mbarrier): a thread announces that its shared-memory writes of a
 // phase are done (arrive, release), goes on with work that needs nobody else's data, and only then
 // waits for the others (acquire).  The three exchanges per plane cost almost no idle issue slots
