@@ -39,7 +39,7 @@ struct Context {
   long long graph_launches = 0;
   int num_sms = 148;
   int stage_ty = MHD_STAGE_TY;  // rows per block of the fused predictor stage (0 = three kernels)
-  bool ct_fused = false;        // corrector CT + face update + CFL as one kernel (slower so far: per-plane barrier)
+  bool ct_fused = false;        // corrector CT + face update + CFL as one kernel (MHD_CT_FUSED=1; 0.81 ms against 0.36 + 0.43)
   int parity = 0;  // flips with every step (which set of face arrays holds B^n)
   // per-launch event timing (mhd_step_profile)
   int prof_n = -1;  // -1 = off, else number of launches recorded so far
@@ -257,7 +257,7 @@ int step_kernels() {
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = c; }
       }
       const int lz = (nz + best - 1) / best;
-      k_ct_update<TY><<<dim3((unsigned)tiles, (nz + lz - 1) / lz), 32 * TY, 0, C.stream>>>(C.U, C.Bnext, C.F, C.Er, g, C.sc, ntx, lz);
+      k_ct_update<TY><<<dim3((unsigned)tiles, (nz + lz - 1) / lz), 32 * TY, CtuTile<TY>::BYTES, C.stream>>>(C.U, C.Bnext, C.F, C.Er, g, C.sc, ntx, lz);
       LAUNCH_CHECK("k_ct_update+cfl");
     } else {
       Box ab, eb;
@@ -349,6 +349,7 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     C.num_sms = sms > 0 ? sms : 148;
+    CU(cudaFuncSetAttribute(k_ct_update<MHD_CTU_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CtuTile<MHD_CTU_TY>::BYTES));
     const char *e = getenv("MHD_STAGE_TY");
     if (e) C.stage_ty = atoi(e);
     e = getenv("MHD_CT_FUSED");
