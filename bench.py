@@ -58,7 +58,10 @@ NCU_TRAFFIC_GB = {1: {"k_predictor_stage": 2.77, "k_flux_x": 2.07, "k_flux_march
                   2: {"k_predictor_stage": 2.85, "k_flux_x": 2.11, "k_flux_march<1>": 2.20,
                       "k_flux_march<2>+update": 4.52, "k_ct(corrector)": 2.14, "k_update(B)+cfl": 1.98}}
 STEP_FLOP_PER_CELL = sum(v[0] for v in KERNEL_MODEL.values())     # 4310 (PLMC; PPMC 4900), algorithmic
-STEP_BYTES_PER_CELL = sum(v[1] for v in KERNEL_MODEL.values())    # 872 as materialised; floor 128
+# what this build executes per active cell and step (ncu, profiles/r2_ncu_kernels.md): flop = dadd + dmul +
+# 2 dfma summed over the step's kernels (halo columns of the stage kernel included); DRAM bytes read + written
+EXECUTED_FLOP_PER_CELL = {1: 3880, 2: 4460}
+NCU_STEP_DRAM_BYTES_PER_CELL = {1: 932, 2: 965}
 
 
 def parse_args():
@@ -71,6 +74,9 @@ def parse_args():
                     help="c1..c5 = BASELINE.json configs[0..4]; or NxNxN[:plmc|ppmc] turbulence cube")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sizes", action="store_true", help="skip the size sweep block (32^3 .. 640^3, PPMC 256^3 / 512^3)")
+    ap.add_argument("--sizes-budget", type=float, default=420.0,
+                    help="wall-clock seconds the size sweep may take; sizes that do not fit are reported as skipped")
     return ap.parse_args()
 
 
@@ -149,11 +155,29 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def time_oracle(problem, n_steps):
-    """The oracle as it stands on the host cores: {compute_dt; step} x n_steps. Returns (cells/s, s)."""
+def time_oracle(problem, n_steps, warmup=0, threads=None):
+    """The oracle as it stands on the host cores: {compute_dt; step} x n_steps.
+    threads=None: all cores, in this process.  threads=k: a child process with OMP_NUM_THREADS=k
+    (the OpenMP runtime reads it once).  Returns (cells/s, seconds, cores)."""
+    nc = problem.n[0] * problem.n[1] * problem.n[2]
+    if threads is not None:
+        code = ("import sys, time, json; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+                "import oracle as orc\nfrom paper_2402_05240_b200 import inputs\n"
+                "p = inputs.turbulence(%d, recon=%d)\n"
+                "o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc); o.set_state(p.state)\n"
+                "t0 = time.perf_counter()\n"
+                "for _ in range(%d): o.step(o.compute_dt(0.4))\n"
+                "print(json.dumps([time.perf_counter() - t0, orc.num_threads()]))\n"
+                % (ROOT, os.path.join(ROOT, "oracle"), problem.n[0], problem.recon, n_steps))
+        env = dict(os.environ, OMP_NUM_THREADS=str(threads))
+        out = subprocess.run([sys.executable, "-c", code], env=env, stdout=subprocess.PIPE, text=True, check=True)
+        el, cores = json.loads(out.stdout.strip().splitlines()[-1])
+        return nc * n_steps / el, el, cores
     import oracle as orc
     o = orc.Oracle(*problem.n, problem.gamma, problem.recon, problem.bc)
     o.set_state(problem.state)
+    for _ in range(warmup):
+        o.step(o.compute_dt(CFL))
     t0 = time.perf_counter()
     for _ in range(n_steps):
         dt = o.compute_dt(CFL)
@@ -161,46 +185,66 @@ def time_oracle(problem, n_steps):
     el = time.perf_counter() - t0
     cores = orc.num_threads()
     o.close()
-    nc = problem.n[0] * problem.n[1] * problem.n[2]
     return nc * n_steps / el, el, cores
 
 
 def sample_problem(workload):
-    """Bounded sample of the workload for the CPU oracle (same recipe, smaller grid where needed)."""
+    """The oracle's workload: the configuration itself where the host can hold it and finish a step in
+    seconds (c1, c2, c3 and 256^3 cubes IN FULL), else a bounded sample of the same recipe."""
     from paper_2402_05240_b200 import inputs
     w = workload.lower()
-    if w in ("c1", "c2"):
+    if w in ("c1", "c2", "c3"):
         p, name = make_problem(w)
-        return p, name + " (full size)"
+        return p, name + " (full size)", True
     if w == "c4":
-        return inputs.blast(64, recon=2), "c4 recipe (blast, PPMC) at 64^3"
+        return inputs.blast(128, recon=2), "c4 recipe (blast, PPMC) at 128^3 (512^3 needs 43 GB and 100 s per step)", False
+    if w == "c5":
+        return inputs.turbulence(256, recon=1), "c5 recipe (Mach-1 beta-1 turbulence, PLMC) at 256^3 (640^3 needs 84 GB)", False
     recon = 2 if w.endswith(":ppmc") else 1
-    return inputs.turbulence(128, recon=recon), "c3/c5 recipe (Mach-1 beta-1 turbulence, recon=%d) at 128^3" % recon
+    n = int(w.split(":")[0].split("x")[0])
+    if n <= 256:
+        p, name = make_problem(w)
+        return p, name + " (full size)", True
+    return inputs.turbulence(256, recon=recon), "turbulence recipe, recon=%d, at 256^3" % recon, False
 
 
 def run_reference(args):
+    """The reference arm of this tier: the CPU oracle, as it stands, on the host cores, on the arm's own
+    workload (c3 in full: 256^3; a step is ~3.5 s on 16 threads).  --steps is honoured up to a wall-clock
+    budget of ~4 minutes; the line says how many steps were timed."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    p, sample = sample_problem(args.workload)
+    p, sample, same = sample_problem(args.workload)
     _, wname = make_problem_name(args.workload)
     import oracle as orc
     o = orc.Oracle(*p.n, p.gamma, p.recon, p.bc)
     o.set_state(p.state)
+    budget = 240.0
+    t_w = time.perf_counter()
+    done_w = 0
     for _ in range(args.warmup):
         o.step(o.compute_dt(CFL))
+        done_w += 1
+        if time.perf_counter() - t_w > 0.15 * budget:
+            break
     t0 = time.perf_counter()
+    done = 0
     for _ in range(args.steps):
         o.step(o.compute_dt(CFL))
+        done += 1
+        if time.perf_counter() - t0 > budget:
+            break
     el = time.perf_counter() - t0
     cores = orc.num_threads()
     o.close()
     nc = p.n[0] * p.n[1] * p.n[2]
-    val = nc * args.steps / el
+    val = nc * done / el
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "steps": done, "warmup": done_w, "ms_per_step": 1e3 * el / done,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": wname, "sample": sample},
+            "data": "synthetic", "config": {"workload": wname, "sample": sample, "same_config": same,
+                                            "steps_requested": args.steps},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -238,6 +282,65 @@ def load_measured_peaks():
         return float(d["hbm_gbs"]), "MEASURED_PEAKS.json"
     except (OSError, KeyError, ValueError):
         return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+SIZES = [("32^3 plmc", "c1"), ("256x16x16 plmc (c2)", "c2"), ("64^3 plmc", "64"), ("128^3 plmc", "128"),
+         ("256^3 ppmc", "256:ppmc"), ("384^3 plmc", "384"), ("512^3 plmc", "512"), ("c4: 512^3 blast ppmc", "c4"),
+         ("c5: 640^3 plmc", "c5")]
+
+
+def size_sweep(mhd, torch, local, budget_s, fp64_tf, flop_cell):
+    """north_star: cell updates/s from 32^3 to 640^3 (PLMC) and for PPMC at 256^3 / 512^3, each with its
+    fraction of the fp64 roofline (counted flop / measured fp64 peak / step time) and the clocks seen."""
+    out, t_start = [], time.perf_counter()
+    for label, w in SIZES:
+        if time.perf_counter() - t_start > budget_s:
+            out.append({"size": label, "skipped": "size-sweep time budget (%.0f s) used up" % budget_s})
+            continue
+        t0 = time.perf_counter()
+        p, _ = make_problem(w)
+        t_gen = time.perf_counter() - t0
+        nc = p.n[0] * p.n[1] * p.n[2]
+        stream = torch.cuda.Stream()
+        try:
+            g = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc, stream=stream)
+        except Exception as e:      # out of memory on a smaller part: reported, not fatal
+            out.append({"size": label, "skipped": "init failed: %s" % str(e)[:80]})
+            continue
+        g.set_state(p.state)
+        steps = 6 if nc >= 300 ** 3 else (12 if nc >= 2 ** 21 else 200)
+        with torch.cuda.stream(stream):
+            g.advance(4 if nc >= 2 ** 21 else 40, CFL)
+            torch.cuda.synchronize()
+            sampler = ClockSampler(local)
+            sampler.start()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = []
+            for _ in range(3):
+                e0.record(stream)
+                g.advance(steps, CFL)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                reps.append(e0.elapsed_time(e1) / steps)
+            clocks = sampler.stop()
+            ok = True
+            try:
+                g.compute_dt(CFL)
+            except mhd.MhdError:
+                ok = False
+        g.close()
+        del g
+        torch.cuda.empty_cache()
+        med = sorted(reps)[1]
+        fc = flop_cell.get(p.recon)
+        out.append({"size": label, "grid": list(p.n), "recon": p.recon, "steps": steps,
+                    "ms_per_step_median": med, "ms_per_step_best": min(reps),
+                    "cell_updates_per_s": nc / (med * 1e-3),
+                    "frac_flop": (fc * nc / (fp64_tf * 1e12)) / (med * 1e-3) if fc else None,
+                    "sm_mhz": clocks.get("sm_mhz"), "power_w_max": clocks.get("power_w_max"),
+                    "reasons": clocks.get("reasons"), "state_ok": ok, "input_gen_s": round(t_gen, 1)})
+        del p
+    return out
 
 
 def run_b200(args):
@@ -283,6 +386,15 @@ def run_b200(args):
         launches = g.launch_count() - l0
         clocks = sampler.stop() if rank == 0 else None
         value, ms = job_value(ms, nc, args.steps, world)
+        # two more regions of the same length (median and best of 3); `value` is the first
+        reps = [ms / args.steps]
+        for _ in range(2):
+            barrier()
+            e0.record(stream)
+            g.advance(args.steps, CFL)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            reps.append(job_value(e0.elapsed_time(e1), nc, args.steps, world)[1] / args.steps)
 
         # ---- per-kernel live timing (CUDA events on the library stream) ----------------
         prof = {}
@@ -355,25 +467,30 @@ def run_b200(args):
                          "frac": hbm_ach / hbm_peak, "peak_source": hbm_src})
             if flop_cell is not None:
                 roof["fp64_achieved_tflops"] = flop_cell * nc / t_top / 1e12
-        # whole-step roofline (north_star): the slower of counted FLOPs at the measured fp64 peak and
-        # the bytes the design moves at the measured HBM bandwidth; the 128 B/cell floor beside it
+        # whole-step roofline (north_star): counted FLOPs at the measured fp64 peak, counted bytes at the
+        # measured HBM bandwidth, and the 128 B/cell floor beside them
         if model:
             step_flop = sum(v[0] for v in model.values())
+            t_step = ms / args.steps * 1e-3
             t_flop = step_flop * nc / (fp64_tf * 1e12)
-            t_byte = STEP_BYTES_PER_CELL * nc / (hbm_peak * 1e9)
-            t_step = ms / args.steps * 1e-3 / 1.0
-            # kernels run one after another, each against its own bound: sum of max(flop, bytes) times
-            t_serial = sum(max(fc * nc / (fp64_tf * 1e12), bc * nc / (hbm_peak * 1e9)) for fc, bc in model.values())
-            roof["step"] = {"flop_per_cell": step_flop, "bytes_per_cell": STEP_BYTES_PER_CELL,
-                            "t_flop_ms": t_flop * 1e3, "t_bytes_ms": t_byte * 1e3,
-                            "frac_of_roofline": max(t_flop, t_byte) / t_step,
-                            "t_serial_ms": t_serial * 1e3, "frac_of_serial_roofline": t_serial / t_step,
+            ex_flop = EXECUTED_FLOP_PER_CELL.get(p.recon)
+            dram = NCU_STEP_DRAM_BYTES_PER_CELL.get(p.recon)
+            roof["step"] = {"flop_per_cell_algorithmic": step_flop, "flop_per_cell_executed": ex_flop,
+                            "dram_bytes_per_cell_ncu": dram,
+                            "frac_flop": t_flop / t_step,
+                            "frac_flop_executed": (ex_flop * nc / (fp64_tf * 1e12)) / t_step if ex_flop else None,
+                            "frac_counted_bytes": (dram * nc / (hbm_peak * 1e9)) / t_step if dram else None,
                             "frac_of_128B_floor": (128.0 * nc / (hbm_peak * 1e9)) / t_step,
-                            "fp64_tflops_step": step_flop * nc / t_step / 1e12}
+                            "fp64_tflops_step_algorithmic": step_flop * nc / t_step / 1e12,
+                            "basis": "algorithmic = dadd + dmul + 2 dfma per active cell of the plain formulation "
+                                     "(round-1 ncu count, profiles/r1_ncu_kernels.md); executed = the same count on "
+                                     "this build (profiles/r2_ncu_kernels.md)"}
         roof["kernels_ms"] = {k: round(v, 4) for k, v in prof.items()}
         roof["measured_here"] = {"fp64_tflops": fp64_tf, "copy_gbs": copy_gbs}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "ms_per_step_repeats": [round(x, 5) for x in reps], "ms_per_step_median": sorted(reps)[1],
+                "ms_per_step_best": min(reps),
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": wname, "grid": list(p.n), "recon": p.recon, "cfl": CFL,
                            "parallelism": "replicas x%d" % world,
@@ -384,11 +501,21 @@ def run_b200(args):
                         "steps": args.e2e_steps},
                 "roofline": roof, "state_ok": not bad_state,
                 "paper_context": {"a100_cell_updates_per_s": 2.59e8, "ratio": value / world / 2.59e8}}
+        if world == 1 and not args.no_sizes:
+            flop_cell = {r: sum(v[0] for v in m.values()) for r, m in MODELS.items()}
+            line["sizes"] = size_sweep(mhd, torch, local, args.sizes_budget, fp64_tf, flop_cell)
         if world == 1 and not args.no_cpu_baseline:
-            sp, sname = sample_problem(args.workload)
-            v, el, cores = time_oracle(sp, 20 if sp.n[0] >= 64 else 400)   # ~10-20 s of host work
+            sp, sname, same = sample_problem(args.workload)
+            big = sp.n[0] * sp.n[1] * sp.n[2] >= 2 ** 22
+            v, el, cores = time_oracle(sp, 5 if big else 200, warmup=1 if big else 5)   # ~20 s of host work
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": sname + ", %.1f s" % el}
+                                    "sample": sname + ", %d steps, %.1f s" % (5 if big else 200, el),
+                                    "same_config": same}
+            if big:   # one thread, labelled: a smaller cube of the same recipe (a 256^3 step takes ~1 min on one core)
+                from paper_2402_05240_b200 import inputs
+                v1, el1, c1 = time_oracle(inputs.turbulence(128, recon=sp.recon), 2, threads=1)
+                line["cpu_baseline"]["single_thread"] = {"value": v1, "cores": c1,
+                                                         "sample": "same recipe at 128^3, 2 steps, %.1f s" % el1}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
