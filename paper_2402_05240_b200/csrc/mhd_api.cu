@@ -39,7 +39,6 @@ struct Context {
   long long graph_launches = 0;
   int num_sms = 148;
   int stage_ty = MHD_STAGE_TY;  // rows per block of the fused predictor stage (0 = three kernels)
-  int stage_cl = MHD_STAGE_CL;  // blocks per cluster of the stage kernel (MHD_STAGE_CL=1 at mhd_init: no clusters)
   bool ct_fused = false;        // corrector CT + face update + CFL as one kernel (MHD_CT_FUSED=1; 0.81 ms against 0.36 + 0.43)
   int parity = 0;  // flips with every step (which set of face arrays holds B^n)
   // per-launch event timing (mhd_step_profile)
@@ -171,14 +170,12 @@ int launch_corrector_fluxes() {
 // Steps 2-5 (PCM + HLLD on cells [-2-r, n+r+1], CT on indices [-1-r, n+r+1], half update of
 // cells [-1-r, n+r]).  MHD_STAGE_TY = 0 runs them as three kernels through the flux arrays,
 // otherwise as the single fused kernel of mhd_stage.cuh with TY rows per block.
-template <int TY, int CL>
+template <int TY>
 int launch_stage_kernel(const Box &hb) {
   const Geo &g = C.g;
-  const int ntx = (hb.hi[0] - hb.lo[0] + 2 + 29) / 30;
-  const int rows = CL * TY - 2;                       // rows owned by one block (CL = 1) or one cluster
-  const int nty = (hb.hi[1] - hb.lo[1] + 2 + rows - 1) / rows;
+  const int ntx = (hb.hi[0] - hb.lo[0] + 2 + 29) / 30, nty = (hb.hi[1] - hb.lo[1] + 2 + TY - 3) / (TY - 2);
   const int nz = hb.hi[2] - hb.lo[2] + 1;
-  const long long tiles = (long long)ntx * nty * CL;  // blocks per z-chunk
+  const long long tiles = (long long)ntx * nty;
   const long long slots = (long long)C.num_sms * (TY <= 8 ? 2 : 1);
   // z is cut into chunks so that the tiles fill the SMs in whole waves; every chunk pays two extra planes
   int best = 1;
@@ -189,23 +186,7 @@ int launch_stage_kernel(const Box &hb) {
   }
   const int lz = (nz + best - 1) / best;
   const size_t smem = (size_t)MHD_STAGE_COLS * 32 * TY * sizeof(double);
-  if (CL == 1) {
-    k_predictor_stage<TY, 1><<<dim3((unsigned)tiles, best), 32 * TY, smem, C.stream>>>(C.U, C.Uh, C.Er, g, hb, C.sc, ntx, lz);
-  } else {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(ntx, nty * CL, best);
-    cfg.blockDim = dim3(32 * TY);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = C.stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 1; attr[0].val.clusterDim.y = CL; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    const Scalars *scp = C.sc;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, k_predictor_stage<TY, CL>, C.U, C.Uh, C.Er, g, hb, scp, ntx, lz);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaLaunchKernelEx(k_predictor_stage)");
-  }
+  k_predictor_stage<TY><<<dim3((unsigned)tiles, best), 32 * TY, smem, C.stream>>>(C.U, C.Uh, C.Er, g, hb, C.sc, ntx, lz);
   LAUNCH_CHECK("k_predictor_stage");
   return MHD_OK;
 }
@@ -215,7 +196,7 @@ int launch_predictor_stage() {
   const int r = recon_radius(g.recon);
   Box hb;
   for (int a = 0; a < 3; a++) { hb.lo[a] = -1 - r; hb.hi[a] = g.n[a] + r; }
-  if (C.stage_ty != 0) return C.stage_cl > 1 ? launch_stage_kernel<MHD_STAGE_TY, MHD_STAGE_CL>(hb) : launch_stage_kernel<MHD_STAGE_TY, 1>(hb);
+  if (C.stage_ty != 0) return launch_stage_kernel<MHD_STAGE_TY>(hb);
   Box pb;
   for (int a = 0; a < 3; a++) { pb.lo[a] = -2 - r; pb.hi[a] = g.n[a] + r + 1; }
   {
@@ -363,8 +344,7 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
   if (!make_geo(g, nx, ny, nz, gamma, recon)) return fail(MHD_ERR_ARG, "mhd_init: bad argument");
   {
     const int cols = MHD_STAGE_COLS * 32 * (int)sizeof(double);
-    CU(cudaFuncSetAttribute(k_predictor_stage<MHD_STAGE_TY, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols * MHD_STAGE_TY));
-    CU(cudaFuncSetAttribute(k_predictor_stage<MHD_STAGE_TY, MHD_STAGE_CL>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols * MHD_STAGE_TY));
+    CU(cudaFuncSetAttribute(k_predictor_stage<MHD_STAGE_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols * MHD_STAGE_TY));
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -372,8 +352,6 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
     CU(cudaFuncSetAttribute(k_ct_update<MHD_CTU_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CtuTile<MHD_CTU_TY>::BYTES));
     const char *e = getenv("MHD_STAGE_TY");
     if (e) C.stage_ty = atoi(e);
-    e = getenv("MHD_STAGE_CL");
-    if (e) C.stage_cl = atoi(e);
     e = getenv("MHD_CT_FUSED");
     if (e) C.ct_fused = atoi(e) != 0;
   }

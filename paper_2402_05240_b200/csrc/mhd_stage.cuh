@@ -23,10 +23,6 @@ namespace mhd {
 #ifndef MHD_STAGE_TY
 #define MHD_STAGE_TY 12
 #endif
-// blocks per cluster along y (1 = no clusters)
-#ifndef MHD_STAGE_CL
-#define MHD_STAGE_CL 4
-#endif
 
 // Split-phase block barrier (mbarrier): a thread announces that its shared-memory writes of a
 // phase are done (arrive, release), goes on with work that needs nobody else's data, and only then
@@ -46,29 +42,6 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned phas
       "r"(phase)
       : "memory");
 }
-
-// Thread-block clusters (sm_90+): CL blocks stacked along y run on CL SMs of one GPC and read each
-// other's shared memory (distributed shared memory), so the row where two of them meet is a row of
-// OWNED cells for both instead of a halo row that both solve: the y halo shrinks from 2 rows in TY to
-// 2 rows in CL * TY.  One hardware barrier per cluster, used split-phase (arrive ... wait) exactly where
-// the single-block version uses its three mbarriers.
-__device__ __forceinline__ unsigned cluster_ctarank() {
-  unsigned r;
-  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-  return r;
-}
-__device__ __forceinline__ unsigned dsm_map(unsigned smem_addr, unsigned rank) {   // same offset in block `rank`
-  unsigned a;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(a) : "r"(smem_addr), "r"(rank));
-  return a;
-}
-__device__ __forceinline__ double dsm_ld(unsigned addr) {
-  double v;
-  asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
-__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
 template <int NT>
 __device__ __forceinline__ void prim_store(double (*P)[NT], int t, const Prim &p) {
@@ -93,9 +66,8 @@ __device__ __forceinline__ F7 stage_face(const Geo &g, const Prim &pm, const Pri
 }
 
 // hb = cells of the half state, [lo, hi] per axis; faces and edges are produced on [lo, hi+1].
-// CL = 1: grid x = tiles (ntx per row of tiles), y = z-chunks of lz planes.
-// CL > 1: clusters of (1, CL, 1) blocks; grid x = tile column, y = CL * (cluster row), z = z-chunk.
-template <int TY, int CL>
+// grid: x = tiles (ntx per row of tiles), y = z-chunks of lz planes.
+template <int TY>
 __global__ void __launch_bounds__(32 * TY, (TY <= 8) ? 2 : 1)
 k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *sc, int ntx, int lz) {
   constexpr int NT = 32 * TY;
@@ -106,38 +78,19 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
   enum { PR = 0, PF = 18, XC = 28, EX = 39, CP = 41, FZ = 49 };
   static_assert(FZ + 5 == MHD_STAGE_COLS, "column count");
   const int t = threadIdx.x, lane = t & 31, row = t >> 5;
-  const int rank = (CL > 1) ? (int)cluster_ctarank() : 0;   // position of this block in its cluster (along y)
-  const int tbx = (CL > 1) ? (int)blockIdx.x : (int)(blockIdx.x % ntx);
-  const int tby = (CL > 1) ? (int)(blockIdx.y / CL) : (int)(blockIdx.x / ntx);
-  const int zch = (CL > 1) ? (int)blockIdx.z : (int)blockIdx.y;
-  const int zc0 = hb.lo[2] + zch * lz, zc1 = min(zc0 + lz - 1, hb.hi[2]);
-  if (zc0 > hb.hi[2]) return;   // (the same for every block of a cluster)
+  const int tbx = blockIdx.x % ntx, tby = blockIdx.x / ntx;
+  const int zc0 = hb.lo[2] + (int)blockIdx.y * lz, zc1 = min(zc0 + lz - 1, hb.hi[2]);
+  if (zc0 > hb.hi[2]) return;
   const int kbeg = zc0 - 1, kend = zc1 + 1;
-  const int i0 = hb.lo[0] + 30 * tbx - 1 + lane, j0 = hb.lo[1] + (CL * TY - 2) * tby - 1 + rank * TY + row;
+  const int i0 = hb.lo[0] + 30 * tbx - 1 + lane, j0 = hb.lo[1] + (TY - 2) * tby - 1 + row;
   // threads beyond the last face index compute on clamped coordinates; nothing of theirs is used
   const int i = min(i0, hb.hi[0] + 1), j = min(j0, hb.hi[1] + 1);
-  const bool low_halo = (rank == 0 && row == 0), high_halo = (rank == CL - 1 && row == TY - 1);
-  const bool own = lane >= 1 && lane <= 30 && !low_halo && !high_halo && i0 <= hb.hi[0] + 1 && j0 <= hb.hi[1] + 1;
+  const bool own = lane >= 1 && lane <= 30 && row >= 1 && row <= TY - 2 && i0 <= hb.hi[0] + 1 && j0 <= hb.hi[1] + 1;
   const bool inx = i0 <= hb.hi[0], iny = j0 <= hb.hi[1];
   const int tl = lane ? t - 1 : t;                  // lower x neighbour (shared memory)
-  // lower / upper y neighbour: the next row of this block, or the facing row of the neighbouring block
-  const int td = row ? t - 32 : (rank > 0 ? t + 32 * (TY - 1) : t);
-  const int tdl = lane ? td - 1 : td;               // lower x, lower y
-  const int tu = (row < TY - 1) ? t + 32 : (rank < CL - 1 ? t - 32 * (TY - 1) : t);
-  const unsigned sm_a = (unsigned)__cvta_generic_to_shared(stage_sm_);
-  unsigned sm_d = sm_a, sm_u = sm_a;                // shared memory that holds the lower / upper neighbour's columns
-  if (CL > 1) {
-    if (row == 0 && rank > 0) sm_d = dsm_map(sm_a, rank - 1);
-    if (row == TY - 1 && rank < CL - 1) sm_u = dsm_map(sm_a, rank + 1);
-  }
-  auto ldd = [&](int col, int idx) -> double {      // column `col`, thread slot `idx` of the lower neighbour's block
-    if (CL > 1) return dsm_ld(sm_d + (unsigned)((col * NT + idx) * 8));
-    return sm[col][idx];
-  };
-  auto ldu = [&](int col, int idx) -> double {
-    if (CL > 1) return dsm_ld(sm_u + (unsigned)((col * NT + idx) * 8));
-    return sm[col][idx];
-  };
+  const int td = row ? t - 32 : t;                  // lower y neighbour
+  const int tdl = (row && lane) ? t - 33 : t;       // lower x, lower y
+  const int tu = (row < TY - 1) ? t + 32 : t;       // upper y neighbour
   const double gm1 = g.gamma - 1.0;
   const double dts = 0.5 * sc->dt;                  // half step (G8)
   const double dtd0 = dts * g.id[0], dtd1 = dts * g.id[1], dtd2 = dts * g.id[2];
@@ -153,12 +106,8 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
     cp_async_commit();
   };
   __shared__ unsigned long long bar[3];
-  if (CL == 1) {
-    if (t == 0) { mbar_init(&bar[0], NT); mbar_init(&bar[1], NT); mbar_init(&bar[2], NT); }
-    __syncthreads();
-  }
-  auto arrive = [&](int b) { if (CL > 1) cluster_arrive(); else mbar_arrive(&bar[b]); };
-  auto wait = [&](int b, unsigned phase) { if (CL > 1) cluster_wait(); else mbar_wait(&bar[b], phase); };
+  if (t == 0) { mbar_init(&bar[0], NT); mbar_init(&bar[1], NT); mbar_init(&bar[2], NT); }
+  __syncthreads();
   prefetch(c);
   double bzl = __ldg(U.f[F_BZ] + c);
   // carried from plane k-1: edge fields, partly updated faces, the cell's hydro variables after
@@ -185,7 +134,7 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
     const double ery = -(pc.v[2] * pc.B[0] - pc.v[0] * pc.B[2]);
     const double erz = -(pc.v[0] * pc.B[1] - pc.v[1] * pc.B[0]);
     sm[XC + 4][t] = erx; sm[XC + 5][t] = erz;
-    arrive(0);
+    mbar_arrive(&bar[0]);
     double Fx0, Fx6, Fy0, Fy5, Fy6, Fz0 = 0.0, Fz5 = 0.0, Fz6 = 0.0;
     if (later) {  // z face (own column only); completes the hydro variables of the cell below
       F7 f = stage_face<2>(g, prim_fetch<NT>(Pp, t), pc, bzl);
@@ -198,7 +147,7 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
       sm[XC + 2][t] = f.m; sm[XC + 3][t] = f.bz;
       Fz0 = f.m; Fz5 = f.by; Fz6 = f.bz;
     }
-    wait(0, ph);   // the neighbours' primitive states are in place
+    mbar_wait(&bar[0], ph);   // the neighbours' primitive states are in place
     {  // x face: Eq. 19 differences in x for this plane's cell
       F7 f = stage_face<0>(g, prim_fetch<NT>(P, tl), pc, bxl);
       accn[0] -= dtd0 * (shfl_dn1(f.m) - f.m);
@@ -210,15 +159,8 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
       Fx0 = f.m; Fx6 = f.bz;
     }
     double Fyh[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    if (!low_halo) {  // y face (the lowest row of a cluster only lends its x and z faces)
-      Prim pd;
-      {
-        const int pcol = PR + 9 * par;
-        pd.rho = ldd(pcol + 0, td); pd.ir = ldd(pcol + 1, td); pd.v[0] = ldd(pcol + 2, td); pd.v[1] = ldd(pcol + 3, td);
-        pd.v[2] = ldd(pcol + 4, td); pd.P = ldd(pcol + 5, td); pd.B[0] = ldd(pcol + 6, td); pd.B[1] = ldd(pcol + 7, td);
-        pd.B[2] = ldd(pcol + 8, td);
-      }
-      F7 f = stage_face<1>(g, pd, pc, byl);
+    if (row > 0) {  // y face (the lowest row only lends its x and z faces)
+      F7 f = stage_face<1>(g, prim_fetch<NT>(P, td), pc, byl);
       Fyh[0] = f.m; Fyh[1] = f.mn; Fyh[2] = f.mt1; Fyh[3] = f.mt2; Fyh[4] = f.e;
       Fy5 = f.by; Fy6 = f.bz;
     } else {
@@ -227,7 +169,7 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
 #pragma unroll
     for (int q = 0; q < 5; q++) sm[XC + 6 + q][t] = Fyh[q];
     Fy0 = Fyh[0];
-    arrive(1);
+    mbar_arrive(&bar[1]);
     // Eq. 15-17 on the three edges at the lower corner of cell (i, j, k); Table 1 signs as in k_ct.
     // E_y needs the x neighbour only (shuffles) ...
     const double ery_l = shfl_up1(ery);
@@ -235,22 +177,22 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
     if (later)
       Ey = ct_edge(-Fz5, -shfl_up1(Fz5), Fx6, sm[CP + 2][t], Fz0, shfl_up1(Fz0), Fx0, sm[CP + 3][t],
                    ery, sm[CP + 5][t], ery_l, sm[CP + 7][t]);
-    wait(1, ph);   // the neighbours' fluxes and reference fields are in place
-    const double erx_d = ldd(XC + 4, td);
+    mbar_wait(&bar[1], ph);   // the neighbours' fluxes and reference fields are in place
+    const double erx_d = sm[XC + 4][td];
     if (later) {  // ... E_x and E_z the row below
-      Ex = ct_edge(-Fy5, -sm[CP + 0][t], Fz6, ldd(XC + 3, td), Fy0, sm[CP + 1][t], Fz0, ldd(XC + 2, td),
+      Ex = ct_edge(-Fy5, -sm[CP + 0][t], Fz6, sm[XC + 3][td], Fy0, sm[CP + 1][t], Fz0, sm[XC + 2][td],
                    erx, erx_d, sm[CP + 4][t], sm[CP + 6][t]);
-      Ez = ct_edge(-sm[XC + 1][t], -ldd(XC + 1, td), Fy6, shfl_up1(Fy6), Fx0, ldd(XC + 0, td), Fy0, shfl_up1(Fy0),
-                   erz, shfl_up1(erz), ldd(XC + 5, td), ldd(XC + 5, tdl));
+      Ez = ct_edge(-sm[XC + 1][t], -sm[XC + 1][td], Fy6, shfl_up1(Fy6), Fx0, sm[XC + 0][td], Fy0, shfl_up1(Fy0),
+                   erz, shfl_up1(erz), sm[XC + 5][td], sm[XC + 5][tdl]);
       sm[EX + 0][t] = Ex; sm[EX + 1][t] = Ez;
     }
-    arrive(2);   // also: nobody reads columns XC+0..5 of another thread beyond this point
+    mbar_arrive(&bar[2]);   // also: nobody reads columns XC+0..5 of another thread beyond this point
     // Eq. 19 differences in y for this plane's cell
-    accn[0] -= dtd1 * (ldu(XC + 6, tu) - Fyh[0]);
-    accn[2] -= dtd1 * (ldu(XC + 7, tu) - Fyh[1]);
-    accn[3] -= dtd1 * (ldu(XC + 8, tu) - Fyh[2]);
-    accn[1] -= dtd1 * (ldu(XC + 9, tu) - Fyh[3]);
-    accn[4] -= dtd1 * (ldu(XC + 10, tu) - Fyh[4]);
+    accn[0] -= dtd1 * (sm[XC + 6][tu] - Fyh[0]);
+    accn[2] -= dtd1 * (sm[XC + 7][tu] - Fyh[1]);
+    accn[3] -= dtd1 * (sm[XC + 8][tu] - Fyh[2]);
+    accn[1] -= dtd1 * (sm[XC + 9][tu] - Fyh[3]);
+    accn[4] -= dtd1 * (sm[XC + 10][tu] - Fyh[4]);
     // this plane's values for the edges of the next one
     sm[CP + 0][t] = Fy5; sm[CP + 1][t] = Fy0; sm[CP + 2][t] = Fx6; sm[CP + 3][t] = Fx0;
     sm[CP + 4][t] = erx; sm[CP + 5][t] = ery; sm[CP + 6][t] = erx_d; sm[CP + 7][t] = ery_l;
@@ -261,9 +203,9 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
     const double Bxh = fma_diff(Bx_part, dtd2, Ey, Ey_p);
     const double Bxuh = shfl_dn1(Bxh);
     const double Eyr = shfl_dn1(Ey), Ezr = shfl_dn1(Ez);
-    wait(2, ph);   // the upper row's edge fields are in place
+    mbar_wait(&bar[2], ph);   // the upper row's edge fields are in place
     if (later) {
-      const double Exu = ldu(EX + 0, tu), Ezu = ldu(EX + 1, tu);
+      const double Exu = sm[EX + 0][tu], Ezu = sm[EX + 1][tu];
       const double Ezur = shfl_dn1(Ezu);
       // Eq. 22: the z face of plane k needs only the edges of this plane
       const double Bzh = fma_diff(fma_diff(bzl, dtd1, Exu, Ex), -dtd0, Eyr, Ey);
@@ -293,7 +235,6 @@ k_predictor_stage(State8 U, State8 Uh, Edge3 Er, Geo g, Box hb, const Scalars *s
     for (int q = 0; q < 5; q++) acc[q] = accn[q];
     bzl = bzu;
   }
-  if (CL > 1) { cluster_arrive(); cluster_wait(); }   // nobody leaves while a neighbour may still read its columns
 }
 
 }  // namespace mhd
