@@ -122,9 +122,10 @@ int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *
 /* Debug/parity: component comp (0 mass, 1 mom_n, 2 mom_t1, 3 mom_t2, 4 energy, 5 B_t1 flux,
  * 6 B_t2 flux; solver-local axes of reading O0) of the corrector HLLD flux on
  * the LOWER `axis`-face of every active cell, as left by the last mhd_step; nx*ny*nz values to a
- * HOST array.  Overwrites the stored half-step state.  Synchronises.  The momentum and energy
- * fluxes of the z sweep (axis 2, comp 1..4) are applied inside the sweep kernel and never stored:
- * MHD_ERR_ARG. */
+ * HOST array.  Synchronises.  Host transfers of every get / set call are staged through a scratch
+ * array of the library's own, so the flux arrays, the half-step state and the state may be read in
+ * any order after a step.  The momentum and energy fluxes of the z sweep (axis 2, comp 1..4) are
+ * applied inside the sweep kernel and never stored: MHD_ERR_ARG. */
 int mhd_get_flux(int axis, int comp, double *out);
 
 /* max over active cells of |sum_a (B_a[upper] - B_a[lower]) / Delta_a|.

@@ -646,6 +646,21 @@ int oracle_get_half_state(double *rho, double *mx, double *my, double *mz, doubl
     return get_any(G.Uh, rho, mx, my, mz, E, bx, by, bz);
 }
 
+/* debug: corrector flux component comp (0 mass, 1 mom_n, 2 mom_t1, 3 mom_t2, 4 energy, 5 B_t1, 6 B_t2;
+ * solver-local order of sweep `axis`) on the lower axis-face of every active cell, as left by the last
+ * step (the predictor's fluxes were overwritten by the corrector's).  Accessor only. */
+int oracle_get_flux(int axis, int comp, double *out)
+{
+    int i, j, k;
+    if (!G.inited) return -2;
+    if (axis < 0 || axis > 2 || comp < 0 || comp > 6 || !out) return -1;
+    for (k = 0; k < G.n[2]; k++)
+        for (j = 0; j < G.n[1]; j++)
+            for (i = 0; i < G.n[0]; i++)
+                out[i + (long)G.n[0] * (j + (long)G.n[1] * k)] = G.F[axis][comp][IDX(&G, i, j, k)];
+    return 0;
+}
+
 /* O1: primitives of one cell, recomputed wherever needed.
  * B_cc from Eq. 13. */
 static void cell_prim(const Grid *g, double *const U[NF], long idx,

@@ -33,6 +33,7 @@ def lib():
         L.oracle_compute_dt.argtypes = [_d, _dp]
         L.oracle_step.argtypes = [_d]
         L.oracle_max_divb.argtypes = [_dp]
+        L.oracle_get_flux.argtypes = [ctypes.c_int, ctypes.c_int, _dp]
         L.oracle_hlld.argtypes = [_d, _dp, _dp, _d, _dp]
         L.oracle_hlld.restype = None
         L.oracle_eigensystem.argtypes = [_d, _dp, _d, _dp, _dp, _dp]
@@ -201,6 +202,14 @@ class Oracle:
         rc = lib().oracle_step(float(dt))
         if rc:
             raise RuntimeError("oracle_step failed: %d" % rc)
+
+    def get_flux(self, axis, comp):
+        nx, ny, nz = self.n
+        out = np.empty((nz, ny, nx))
+        rc = lib().oracle_get_flux(int(axis), int(comp), _p(out))
+        if rc:
+            raise RuntimeError("oracle_get_flux failed: %d" % rc)
+        return out
 
     def max_divb(self):
         v = ctypes.c_double()

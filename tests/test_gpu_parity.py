@@ -379,6 +379,30 @@ def test_error_codes(mhd):
     g.close()
 
 
+@pytest.mark.parametrize("recon", [1, 2])
+def test_corrector_fluxes_against_oracle(mhd, recon):
+    """mhd_get_flux: the corrector (Step 7) flux components that the library keeps in
+    memory -- all seven of the x and y sweeps, mass and the two induction components of the z sweep (its
+    momentum / energy fluxes are consumed in the sweep) -- against the oracle's, face by face; the call
+    is made after mhd_get_state, which must not disturb them (host I/O is staged elsewhere)."""
+    p = inputs.random_smooth(n=(37, 21, 19), seed=31, recon=recon)
+    o, g = make_pair(mhd, p)
+    dt = o.compute_dt(p.cfl)
+    o.step(dt); g.step(dt)
+    g.get_state()
+    for axis in range(3):
+        ref = {c: o.get_flux(axis, c) for c in range(7)}
+        scale = max(np.abs(r).max() for r in ref.values())
+        for c in range(7):
+            if axis == 2 and 1 <= c <= 4:
+                with pytest.raises(mhd.MhdError):
+                    g.get_flux(axis, c)
+                continue
+            got = g.get_flux(axis, c)
+            assert np.abs(got - ref[c]).max() <= TOL_STEP * scale, (axis, c)
+    o.close(); g.close()
+
+
 def test_unphysical_flag_belongs_to_the_state_it_was_computed_on(mhd):
     """MHD_ERR_UNPHYSICAL is not sticky: after a bad state, mhd_set_state(good) + mhd_compute_dt
     succeeds (PAPER.md:523 on error reporting; SURVEY.md 8(b) error convention)."""
