@@ -9,6 +9,7 @@
 #include "mhd_kernels.cuh"
 #include "mhd_stage.cuh"
 #include "mhd_ctupdate.cuh"
+#include "mhd_small.cuh"
 
 using namespace mhd;
 
@@ -39,6 +40,11 @@ struct Context {
   long long graph_launches = 0;
   int num_sms = 148;
   int stage_ty = MHD_STAGE_TY;  // rows per block of the fused predictor stage (0 = three kernels)
+  // launch-bound grids: the whole of mhd_advance as one cooperative kernel (mhd_small.cuh).
+  // 0 = mhd_advance on grids of at most MHD_SMALL_MAX_CELLS cells; 1 = mhd_step too, any size (MHD_SMALL=1
+  // at mhd_init: parity tests); -1 = never (MHD_SMALL=0)
+  int small_mode = 0;
+  bool coop = false;
   bool ct_fused = false;        // corrector CT + face update + CFL as one kernel (MHD_CT_FUSED=1; 0.81 ms against 0.36 + 0.43)
   int parity = 0;  // flips with every step (which set of face arrays holds B^n)
   // per-launch event timing (mhd_step_profile)
@@ -49,6 +55,7 @@ struct Context {
 
 Context C;
 char g_err[512] = "no error";
+int run_small(int n_steps, double cfl, double dt_fixed);
 
 int fail(int code, const char *msg) {
   snprintf(g_err, sizeof(g_err), "%s", msg);
@@ -352,6 +359,11 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
     CU(cudaFuncSetAttribute(k_ct_update<MHD_CTU_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CtuTile<MHD_CTU_TY>::BYTES));
     const char *e = getenv("MHD_STAGE_TY");
     if (e) C.stage_ty = atoi(e);
+    e = getenv("MHD_SMALL");
+    if (e) C.small_mode = atoi(e) ? 1 : -1;
+    int coop = 0;
+    CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    C.coop = coop != 0;
     e = getenv("MHD_CT_FUSED");
     if (e) C.ct_fused = atoi(e) != 0;
   }
@@ -420,6 +432,61 @@ int get_state_to(State8 &S, double *const dst[NFIELD], bool host) {
     LAUNCH_CHECK("k_pack");
     if (host) CU(cudaMemcpyAsync(dst[f], ddst, cnt * sizeof(double), cudaMemcpyDeviceToHost, C.stream));
   }
+  return MHD_OK;
+}
+
+#ifndef MHD_SMALL_MAX_CELLS
+#define MHD_SMALL_MAX_CELLS (1LL << 15)   // 32^3: measured 62 against 79 us per step; 64^3 is a tie, 256 x 16 x 16 loses
+#endif
+
+template <int RC>
+int launch_small(SmallArgs &a) {
+  static int blocks_per_sm = -1;
+  if (blocks_per_sm < 0) {
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, k_small_steps<RC>, 256, 0));
+    if (blocks_per_sm < 1) return fail(MHD_ERR_CUDA, "k_small_steps does not fit on an SM");
+  }
+  const Geo &g = C.g;
+  const int r = recon_radius(RC);
+  long long work = 1;
+  for (int x = 0; x < 3; x++) work *= (g.n[x] + 2 * r + 4);   // the largest phase: predictor fluxes
+  long long blocks = (work + 255) / 256;
+  const long long cap = (long long)blocks_per_sm * C.num_sms;   // co-resident blocks (grid barrier)
+  if (blocks > cap) blocks = cap;
+  void *args[] = {&a};
+  CU(cudaLaunchCooperativeKernel((void *)k_small_steps<RC>, dim3((unsigned)blocks), dim3(256), args, 0, C.stream));
+  LAUNCH_CHECK("k_small_steps");
+  return MHD_OK;
+}
+
+// n steps of { dt = cfl / max rate (or dt_fixed); step } in one cooperative launch
+int run_small(int n_steps, double cfl, double dt_fixed) {
+  SmallArgs a;
+  a.U = C.U; a.Uh = C.Uh; a.F = C.F; a.E = C.E; a.Er = C.Er; a.Bnext = C.Bnext; a.g = C.g; a.sc = C.sc;
+  a.n_steps = n_steps; a.cfl = cfl; a.dt_fixed = dt_fixed;
+  a.dbg = getenv("MHD_SMALL_DEBUG") ? (unsigned long long *)C.scratch : nullptr;
+  int rc;
+  switch (C.g.recon) {
+    case 0: rc = launch_small<0>(a); break;
+    case 1: rc = launch_small<1>(a); break;
+    case 2: rc = launch_small<2>(a); break;
+    case 3: rc = launch_small<3>(a); break;
+    default: rc = launch_small<4>(a); break;
+  }
+  if (rc) return rc;
+  if (a.dbg) {
+    unsigned long long h[16];
+    cudaMemcpyAsync(h, a.dbg, sizeof(h), cudaMemcpyDeviceToHost, C.stream);
+    cudaStreamSynchronize(C.stream);
+    fprintf(stderr, "k_small_steps last step, us per phase (ghosts, pred flux, ct, half update, face flux, ct, update):");
+    for (int q = 1; q < 8; q++) fprintf(stderr, " %.1f", (h[q] - h[q - 1]) * 1e-3);
+    fprintf(stderr, "\n");
+  }
+  if (n_steps & 1) {   // the B ping-pong inside the kernel ended on the other set of face arrays
+    for (int x = 0; x < 3; x++) { double *t = C.Bnext.f[x]; C.Bnext.f[x] = C.U.f[F_BX + x]; C.U.f[F_BX + x] = t; }
+    C.parity ^= 1;
+  }
+  C.rate_valid = true;
   return MHD_OK;
 }
 
@@ -504,6 +571,7 @@ int mhd_compute_dt(double cfl, double *dt) {
 int mhd_step(double dt) {
   if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
   if (!(dt > 0.0)) return fail(MHD_ERR_ARG, "mhd_step: dt must be positive");
+  if (C.small_mode == 1 && C.coop && C.prof_n < 0) return run_small(1, 1.0, dt);
   k_set_dt<<<1, 1, 0, C.stream>>>(C.sc, dt);
   LAUNCH_CHECK("k_set_dt");
   return step_kernels();
@@ -521,7 +589,14 @@ int mhd_advance(int n_steps, double cfl, double *t_accum) {
   }
   int s = 0;
   const long long ncell = (long long)C.g.n[0] * C.g.n[1] * C.g.n[2];
-  if (C.stream != 0 && n_steps >= 4 && ncell <= (1LL << 21) && C.prof_n < 0) {  // launch-bound sizes only
+  if (C.coop && C.prof_n < 0 && n_steps > 0 && (C.small_mode == 1 || (C.small_mode == 0 && ncell <= MHD_SMALL_MAX_CELLS))) {
+    int rc = ensure_rate();
+    if (rc) return rc;
+    rc = run_small(n_steps, cfl, 0.0);
+    if (rc) return rc;
+    s = n_steps;
+  }
+  if (C.stream != 0 && n_steps - s >= 4 && ncell <= (1LL << 21) && C.prof_n < 0) {  // launch-bound sizes only
     int rc = ensure_rate();
     if (rc) return rc;
     const int p = C.parity;

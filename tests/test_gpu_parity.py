@@ -293,9 +293,10 @@ def test_c3_turbulence_small_multi_step(mhd):
     o.close(); g.close()
 
 
-def test_advance_matches_stepwise_and_device_io(mhd):
+def test_advance_matches_stepwise_and_device_io(mhd, monkeypatch):
     """mhd_advance (dt kept on the device) == {compute_dt; step} loop; device set/get == host set/get."""
     import torch
+    monkeypatch.setenv("MHD_SMALL", "0")                # the kernel-by-kernel path (bitwise comparison below)
     p = inputs.random_smooth(n=(40, 24, 18), seed=8, recon=1)
     g = mhd.Mhd(*p.n, p.gamma, p.recon)
     g.set_state(p.state)
@@ -317,11 +318,12 @@ def test_advance_matches_stepwise_and_device_io(mhd):
 
 
 @pytest.mark.parametrize("recon,bc", [(1, (0, 0, 0)), (2, (1, 0, 0))])
-def test_advance_graph_path_is_bitwise_the_stepwise_path(mhd, recon, bc):
+def test_advance_graph_path_is_bitwise_the_stepwise_path(mhd, recon, bc, monkeypatch):
     """On a non-default stream and a small grid mhd_advance replays a CUDA graph of two steps; an odd
     step count, a second call (other orientation of the B ping-pong) and a boundary change in between
     must all give exactly what the kernel-by-kernel path gives."""
     import torch
+    monkeypatch.setenv("MHD_SMALL", "0")                # (a grid this small would take the cooperative kernel)
     p = inputs.random_smooth(n=(33, 20, 17), seed=12, recon=recon)
     ref = mhd.Mhd(*p.n, p.gamma, p.recon, bc)           # default stream: no graph
     ref.set_state(p.state)
