@@ -471,8 +471,9 @@ def test_full_size_sampled_parity(mhd, workload):
     advanced by the oracle as a small periodic box with dt scaled by N/m = 16 (ideal MHD has no
     length scale; the factor is a power of two, so dt/Delta is the same number bit for bit); one
     step reaches at most 7 cells, so the block's interior (8 cells from its rim) is exact and must
-    match the GPU's full-grid result to 1e-12.  Two consecutive steps are checked, each from the
-    GPU's own state, plus div B and positivity on the whole grid."""
+    match the GPU's full-grid result to 1e-12.  Steps 1, 2, the middle and the last step of the
+    config's run (20 for c4, 10 for c5) are checked, each from the GPU's own state before it, plus
+    div B and positivity on the whole grid."""
     if workload == "c4":
         p = inputs.blast(512, recon=2)
         N, m = 512, 32
@@ -487,9 +488,20 @@ def test_full_size_sampled_parity(mhd, workload):
     g.set_state(p.state)
     before = p.state
     worst = 0.0
-    for step in range(2):
+    # the config's own step count (c4: 20, c5: 10): steps 1, 2, the middle one and the last one are
+    # checked, each from the GPU's own state before it; the steps in between run through mhd_advance
+    nsteps = 20 if workload == "c4" else 10
+    done = 0
+    for step in (1, 2, nsteps // 2, nsteps):
+        if step - 1 > done:
+            g.advance(step - 1 - done, p.cfl)
+            done = step - 1
+            p.state = None                      # (host memory: at most two full states at a time)
+            before = after = None
+            before = g.get_state()
         dt = g.compute_dt(p.cfl)
         g.step(dt)
+        done += 1
         after = g.get_state()
         assert np.min(after["rho"]) > 0.0 and np.all(np.isfinite(after["E"]))
         for org in orgs:
@@ -506,7 +518,7 @@ def test_full_size_sampled_parity(mhd, workload):
                     max(np.abs(before["rho"]).max(), 1e-300)
                 d = np.abs(a - b).max() / scale
                 worst = max(worst, d)
-                assert d <= TOL_STEP, "%s step %d block %s field %s: %.3e" % (workload, step + 1, org, f, d)
+                assert d <= TOL_STEP, "%s step %d block %s field %s: %.3e" % (workload, step, org, f, d)
         before = after
     assert g.max_divb() * (1.0 / N) / np.sqrt(np.mean(before["bx"] ** 2 + 0) * 3) <= TOL_DIVB
     g.close()
