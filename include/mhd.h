@@ -128,6 +128,12 @@ int mhd_get_half_state(double *rho, double *mx, double *my, double *mz, double *
  * applied inside the sweep kernel and never stored: MHD_ERR_ARG. */
 int mhd_get_flux(int axis, int comp, double *out);
 
+/* Debug layout check.  With MHD_GUARD=1 in the environment at mhd_workspace_bytes / mhd_init time every
+ * array of the context sits between guard bands filled with a NaN pattern and itself starts as that pattern;
+ * *n_bad receives the number of guard words that no longer hold it (0 = no kernel has written outside its
+ * arrays), or -1 if the context is not guarded.  Synchronous; *n_bad is a HOST pointer. */
+int mhd_debug_guard_errors(long long *n_bad);
+
 /* max over active cells of |sum_a (B_a[upper] - B_a[lower]) / Delta_a|.
  * Synchronous; *out is a HOST pointer. */
 int mhd_max_divb(double *out);

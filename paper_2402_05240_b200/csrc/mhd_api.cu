@@ -29,6 +29,7 @@ struct Context {
   Edge3 Er;  // cell-centred reference field, Eq. 18
   Edge3 Bnext;  // face arrays that receive B^{n+1}; swapped with U's after every step
   double *scratch = nullptr;  // staging of the host set/get calls (never a result array)
+  size_t guard = 0;           // bytes of the guard band on either side of every array (MHD_GUARD=1), else 0
   Scalars *sc = nullptr;
   cudaStream_t stream = 0;
   long long launches = 0;
@@ -107,7 +108,34 @@ const int kNumArrays = 2 * NFIELD + 21 + 3 + 3 + 3 + 1;  // U, half state, fluxe
 
 size_t array_bytes(const Geo &g) { return ((size_t)g.ntot * sizeof(double) + 255) / 256 * 256; }
 
-size_t total_bytes(const Geo &g) { return array_bytes(g) * kNumArrays + 256; }
+// Debug layout (MHD_GUARD=1 in the environment of mhd_workspace_bytes / mhd_init): every array sits between
+// two guard bands of four z-planes filled with a NaN pattern, and the arrays themselves start as that
+// pattern instead of zero.  A write outside an array lands in a guard band (mhd_debug_guard_errors counts
+// the damaged words), a read outside it or of a never-written element yields NaN, which surfaces in the
+// parity tests if it reaches a result.  compute-sanitizer is closed on this GPU pool; this is the check
+// the library carries itself.
+const unsigned long long kGuardPattern = 0x7ff8dead0badf00dull;
+size_t guard_bytes(const Geo &g) {
+  const char *e = getenv("MHD_GUARD");
+  if (!e || !atoi(e)) return 0;
+  return ((size_t)4 * g.s[2] * sizeof(double) + 255) / 256 * 256;
+}
+
+size_t total_bytes(const Geo &g) { return (array_bytes(g) + 2 * guard_bytes(g)) * kNumArrays + 256; }
+
+__global__ void k_fill_pattern(unsigned long long *p, size_t n, unsigned long long v) {
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) p[t] = v;
+}
+// words of the guard bands (slots of `slot` words: guard | array | guard) that no longer hold the pattern
+__global__ void k_count_guard_damage(const unsigned long long *p, size_t slot, size_t guard, int nslots,
+                                     unsigned long long v, unsigned long long *count) {
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < (size_t)nslots * 2 * guard;
+       t += (size_t)gridDim.x * blockDim.x) {
+    const size_t s_ = t / (2 * guard), w = t % (2 * guard);
+    const size_t off = s_ * slot + (w < guard ? w : slot - 2 * guard + w);
+    if (p[off] != v) atomicAdd(count, 1ull);
+  }
+}
 
 dim3 grid1(long long n, int block) { return dim3((unsigned)((n + block - 1) / block)); }
 
@@ -379,8 +407,11 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
   C.bytes = need;
   C.g = g;
   char *p = (char *)C.base;
-  size_t ab = array_bytes(g);
+  const size_t gb = guard_bytes(g);
+  const size_t ab = array_bytes(g) + 2 * gb;   // one slot: guard | array | guard
+  C.guard = gb;
   C.sc = (Scalars *)p; p += 256;
+  p += gb;                                     // array pointers point past the leading guard
   for (int f = 0; f < NFIELD; f++) { C.U.f[f] = (double *)p; p += ab; }
   for (int f = 0; f < NFIELD; f++) { C.Uh.f[f] = (double *)p; p += ab; }
   for (int a = 0; a < 3; a++)
@@ -394,6 +425,10 @@ int init_common(int nx, int ny, int nz, double gamma, int recon, void *ws, size_
   C.inited = true;
   cudaError_t e = cudaMemsetAsync(C.base, 0, need, C.stream);
   if (e != cudaSuccess) { mhd_finalize(); return cuda_fail(e, "cudaMemsetAsync"); }
+  if (gb) {   // guards AND arrays start as the NaN pattern (the scalars stay zero)
+    k_fill_pattern<<<1024, 256, 0, C.stream>>>((unsigned long long *)((char *)C.base + 256), (need - 256) / 8, kGuardPattern);
+    LAUNCH_CHECK("k_fill_pattern");
+  }
   k_reset_rate<<<1, 1, 0, C.stream>>>(C.sc);
   LAUNCH_CHECK("k_reset_rate");
   return MHD_OK;
@@ -716,6 +751,24 @@ int mhd_step_profile(double dt, int max_entries, double *ms, const char **names,
   }
   for (int i = 0; i <= kMaxProf; i++) cudaEventDestroy(C.prof_ev[i]);
   return rc;
+}
+
+int mhd_debug_guard_errors(long long *n_bad) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (!n_bad) return fail(MHD_ERR_ARG, "mhd_debug_guard_errors: null pointer");
+  *n_bad = -1;
+  if (!C.guard) return MHD_OK;   // not a guarded context
+  unsigned long long *cnt = (unsigned long long *)&C.sc[1];   // (the scalar block is 256 bytes)
+  CU(cudaMemsetAsync(cnt, 0, sizeof(*cnt), C.stream));
+  const size_t slot = (array_bytes(C.g) + 2 * C.guard) / 8;
+  k_count_guard_damage<<<512, 256, 0, C.stream>>>((const unsigned long long *)((char *)C.base + 256), slot, C.guard / 8,
+                                                  kNumArrays, kGuardPattern, cnt);
+  LAUNCH_CHECK("k_count_guard_damage");
+  unsigned long long h = 0;
+  CU(cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, C.stream));
+  CU(cudaStreamSynchronize(C.stream));
+  *n_bad = (long long)h;
+  return MHD_OK;
 }
 
 long long mhd_launch_count(void) { return C.launches; }

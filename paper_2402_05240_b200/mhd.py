@@ -59,6 +59,8 @@ def _load():
     L.mhd_unit_reconstruct.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_int, _dp, _dp, _dp, _dp]
     L.mhd_unit_ct_edge.argtypes = [ctypes.c_int, _dp, _dp]
     L.mhd_unit_math.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp]
+    L.mhd_debug_guard_errors.argtypes = [ctypes.POINTER(ctypes.c_longlong)]
+    L.mhd_debug_guard_errors.restype = ctypes.c_int
     L.mhd_launch_count.restype = ctypes.c_longlong
     L.mhd_last_error.restype = ctypes.c_char_p
     for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_domain", "mhd_set_stream", "mhd_set_state",
@@ -237,6 +239,12 @@ class Mhd:
         out = np.empty((self.n[2], self.n[1], self.n[0]))
         _check(_lib.mhd_get_flux(int(axis), int(comp), _hp(out)))
         return out
+
+    def guard_errors(self):
+        """Damaged guard words of a context created with MHD_GUARD=1 (-1: not a guarded context)."""
+        n = ctypes.c_longlong()
+        _check(_lib.mhd_debug_guard_errors(ctypes.byref(n)))
+        return n.value
 
     def max_divb(self):
         v = ctypes.c_double()
