@@ -567,6 +567,7 @@ __global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM :
   };
   W7 W0c, dLc;
   double bn0c = 0.0;
+  [[maybe_unused]] double bface = 0.0, bface_next = 0.0;   // normal field on faces f, f+1 (PLM: from the prefetched cells)
   if constexpr (PLM) {
     double bnm;
     const W7 Wm = to_W<A>(load_prim_half(Uh, g, idx - 2 * sA), bnm);
@@ -628,11 +629,9 @@ __global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM :
       p.B[0] = 0.5 * (pre[b][5][tid] + pre[b][6][tid]);
       p.B[1] = 0.5 * (pre[b][7][tid] + pre[b][8][tid]);
       p.B[2] = 0.5 * (pre[b][9][tid] + pre[b][10][tid]);
-#ifdef MHD_EXP_NOLOAD
-      if (f < fend) prefetch(b ^ 1, idx - (long long)(f - f0) * sA);
-#else
+      bface = bface_next;                        // face f: the lower A-face of cell f, seen one iteration ago
+      bface_next = pre[b][5 + 2 * A][tid];       // lower A-face of the entering cell f+1 = face f+1
       if (f < fend) prefetch(b ^ 1, idx + (long long)(R + 1) * sA);
-#endif
       cp_async_commit();
       double bnp;
       const W7 Wp = to_W<A>(p, bnp);
@@ -655,11 +654,8 @@ __global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM :
       reconstruct<RC>(g.gamma, win, bnc[R], lo, hi);
     }
     if (f >= f0) {
-      F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, __ldg(Uh.f[F_BX + A] + idx));
+      F7 fl = hlld(g.gamma, g.gm1inv, WL, lo, PLM ? bface : __ldg(Uh.f[F_BX + A] + idx));
       if (!UPDATE) {
-#ifdef MHD_EXP_NOSTORE
-        if (fl.m == 12345.678)
-#endif
         store_flux<A>(F, idx, fl);
       } else {
         if (f <= f1) { F.f[A][0][idx] = fl.m; F.f[A][5][idx] = fl.by; F.f[A][6][idx] = fl.bz; }
