@@ -15,27 +15,23 @@
 
 namespace mhd {
 
-// 1/x for normal x.
+// 1/x for normal x.  One step of the cubically convergent iteration y <- y (1 + e + e^2), e = 1 - x y:
+// the seed's relative error of < 2^-20 goes to e^3 < 2^-60, below the rounding of the last FMA.
 __device__ __forceinline__ double rcp(double x) {
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   double e = __fma_rn(-x, y, 1.0);
-  y = __fma_rn(y, e, y);
-  e = __fma_rn(-x, y, 1.0);
-  y = __fma_rn(y, e, y);
-  return y;
+  double t = __fma_rn(e, e, e);
+  return __fma_rn(y, t, y);
 }
 
-// 1/sqrt(x) for normal x > 0.
+// 1/sqrt(x) for normal x > 0.  Cubic step y <- y (1 + e/2 + 3 e^2/8), e = 1 - x y^2 (remainder 5 e^3/16).
 __device__ __forceinline__ double rsqrt_(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double h = 0.5 * x;
-  double e = __fma_rn(-h * y, y, 0.5);   // 1/2 - x y^2 / 2
-  y = __fma_rn(y, e, y);
-  e = __fma_rn(-h * y, y, 0.5);
-  y = __fma_rn(y, e, y);
-  return y;
+  double e = __fma_rn(-(x * y), y, 1.0);
+  double t = __fma_rn(0.375, e, 0.5) * e;
+  return __fma_rn(y, t, y);
 }
 
 // sqrt(x) for normal x > 0, and exactly 0 for x == 0 (x < 0 is the caller's bug).  One Newton step
