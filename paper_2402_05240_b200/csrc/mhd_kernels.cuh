@@ -263,7 +263,7 @@ __device__ __forceinline__ void pcm_face(double (*st)[MHD_PRED_T], const State8 
 #define MHD_MINB_FX 5
 #endif
 #ifndef MHD_MINB_FM
-#define MHD_MINB_FM 4
+#define MHD_MINB_FM 3
 #endif
 #ifndef MHD_MINB_FMZ
 #define MHD_MINB_FMZ 3
