@@ -165,6 +165,11 @@ Box make_box(int l0, int h0, int l1, int h1, int l2, int h2) {
   return b;
 }
 
+// cells per thread of a marching sweep (each chunk reconstructs one cell more than it solves faces)
+#ifndef MHD_MARCH_J
+#define MHD_MARCH_J 32
+#endif
+
 template <int RC>
 int launch_corrector_fluxes() {
   const Geo &g = C.g;
@@ -181,10 +186,7 @@ int launch_corrector_fluxes() {
   }
   {
     Box fb = make_box(-1, n0, 0, n1, -1, n2);
-    int J = (n1 + 1 >= 64) ? 32 : ((n1 + 1 >= 16) ? 8 : 4);
-#ifdef MHD_FORCE_J
-    J = MHD_FORCE_J;
-#endif
+    int J = (n1 + 1 >= 2 * MHD_MARCH_J) ? MHD_MARCH_J : ((n1 + 1 >= 16) ? 8 : 4);
     long long nt = (long long)(n0 + 2) * (n2 + 2);
     dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
     k_flux_march<1, RC, false><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
@@ -192,7 +194,7 @@ int launch_corrector_fluxes() {
   }
   {
     Box fb = make_box(-1, n0, -1, n1, 0, n2);
-    int J = (n2 + 1 >= 64) ? 32 : ((n2 + 1 >= 16) ? 8 : 4);
+    int J = (n2 + 1 >= 2 * MHD_MARCH_J) ? MHD_MARCH_J : ((n2 + 1 >= 16) ? 8 : 4);
     long long nt = (long long)(n0 + 2) * (n1 + 2);
     dim3 grid(grid1(nt, 128).x, (n2 + 1 + J - 1) / J);
     k_flux_march<2, RC, true><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
