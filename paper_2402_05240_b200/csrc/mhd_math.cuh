@@ -5,10 +5,13 @@
 // branch bookkeeping each, and the step executes ~110 of them per cell.  Every operand here is a
 // physical quantity of ordinary magnitude (densities, speeds, pressures; never denormal, never
 // near overflow), so the slow path is dead weight.  These versions take the same hardware seed
-// (MUFU.RCP64H / MUFU.RSQ64H through PTX rcp.approx / rsqrt.approx, relative error < 2^-22) and
-// two Newton steps in fp64 FMAs (error -> 2^-44 -> rounding level).  The results are within 1 ulp
-// of the correctly rounded value: this is full fp64 precision, not -use_fast_math (which would
-// not touch fp64 anyway); the parity tolerance (1e-12) is four orders of magnitude looser.
+// (MUFU.RCP64H / MUFU.RSQ64H through PTX rcp.approx / rsqrt.approx, relative error < 2^-20) and
+// ONE step of a cubically convergent iteration in fp64 FMAs (error e -> ~e^3 < 2^-60, below the
+// rounding of the last FMA): 3 fp64 instructions for 1/x, 5 for 1/sqrt(x), 6 for sqrt(x), each a
+// dependent chain of 3-4 (two Newton steps were 4 / 7 / 8 instructions and chains of 4-7).  The
+// results are within 2 ulp of the correctly rounded value (tests/test_gpu_units.py, 200 000 operands
+// over 60 decades): full fp64 precision, not -use_fast_math (which would not touch fp64 anyway);
+// the parity tolerance (1e-12) is four orders of magnitude looser.
 // Not valid for 0, denormal, infinite or NaN operands beyond what is noted per function.
 #pragma once
 #include <cuda_runtime.h>
