@@ -259,7 +259,11 @@ int launch_predictor_stage() {
 int step_kernels() {
   const Geo &g = C.g;
   const int r = recon_radius(g.recon);
-  int rc = fill_ghosts(C.U);  // one boundary update per step
+  // One boundary update per step.  k_predictor_stage, the only reader of U^n outside the
+  // active cells, applies the boundary map to its own loads (mhd_stage.cuh): the ghost layers are then
+  // filled only by mhd_set_state; the three-kernel predictor reads filled layers.
+  int rc = MHD_OK;
+  if (C.stage_ty == 0) rc = fill_ghosts(C.U);
   if (rc) return rc;
   rc = launch_predictor_stage();
   if (rc) return rc;

@@ -514,6 +514,14 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) 
 }
 
 #define MHD_WSM_BYTES (5 * 8 * 128 * 8)
+// the PLM y march is unrolled by two: the carried cell, difference and face state (24 doubles) then change
+// names instead of registers (45 moves less per iteration; 0.715 -> 0.696 ms at 256^3); the z march with the
+// update loses with it (0.88 -> 0.92 ms)
+#ifndef MHD_MARCH_UNROLL
+#define MHD_MARCH_UNROLL 2
+#endif
+#define MHD_PRAGMA_(x) _Pragma(#x)
+#define MHD_UNROLL(n) MHD_PRAGMA_(unroll n)
 // y / z sweep: a thread owns one x position (warps run along x, so every load and store is
 // coalesced) and marches along the sweep axis over a chunk of J faces with a rolling window
 // of 2R+1 primitive states in registers; each cell's primitives are formed once per chunk.
@@ -618,6 +626,7 @@ __global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM :
   // One reconstruct() call site per kernel: iteration f0-1 only produces W_L of face f0; every
   // cell is then reconstructed by the same instruction sequence, so mirror-image cells give
   // mirror-image states bit for bit.
+  MHD_UNROLL((PLM && !UPDATE) ? MHD_MARCH_UNROLL : 1)
   for (int f = f0 - 1; f <= fend; f++, idx += sA) {
     if constexpr (PLM) {
       cp_async_wait_but_last();  // the prefetch of cell f+1 (the newer group is the update's)

@@ -93,7 +93,7 @@ def test_fused_predictor_stage_agrees_with_the_three_kernel_path(mhd, recon, n, 
         g.step(g.compute_dt(p.cfl))
         out[ty] = (g.get_half_state(), g.get_state(), g.launch_count() - n0)
         g.close()
-    assert out["0"][2] - out["12"][2] == 2               # three launches became one
+    assert out["0"][2] - out["12"][2] == 3               # ghost fill + three launches became one
     assert_close(out["12"][0], out["0"][0], 1e-13, "half state, fused vs three kernels")
     assert_close(out["12"][1], out["0"][1], 1e-13, "full state, fused vs three kernels")
 
