@@ -165,10 +165,33 @@ Box make_box(int l0, int h0, int l1, int h1, int l2, int h2) {
   return b;
 }
 
-// cells per thread of a marching sweep (each chunk reconstructs one cell more than it solves faces)
+// Faces per thread of a marching sweep.  A chunk costs its faces plus `extra` iterations (the cell it
+// reconstructs without solving a face, the start-up loads; the z sweep also solves one face of the next
+// chunk), and the grid should fill the SMs' block slots in whole waves: with few waves (<= 128^3) the
+// quantisation decides, with many (>= 256^3) the start-up share does and J ~ 32 is the measured optimum.
 #ifndef MHD_MARCH_J
 #define MHD_MARCH_J 32
 #endif
+
+int march_chunk(int nfaces, long long blocks_per_chunk, int extra) {
+  const double slots = (double)C.num_sms * MHD_MINB_FM;
+  const int n32 = (nfaces + MHD_MARCH_J - 1) / MHD_MARCH_J;
+  if ((double)(blocks_per_chunk * n32) > 6.0 * slots) {   // many waves: even chunks of about MHD_MARCH_J
+    const int nch = (nfaces + MHD_MARCH_J / 2) / MHD_MARCH_J;
+    return (nfaces + nch - 1) / nch;
+  }
+  int best = nfaces;
+  double best_cost = -1.0;
+  for (int J = nfaces < 4 ? nfaces : 4; J <= nfaces && J <= 2 * MHD_MARCH_J; J++) {
+    const int nch = (nfaces + J - 1) / J;
+    if ((nfaces + nch - 1) / nch != J) continue;   // even chunks only
+    const double waves = (double)(blocks_per_chunk * nch) / slots;
+    const double rounds = (waves <= 4.0) ? ceil(waves) : waves + 0.5;
+    const double cost = rounds * (J + extra);
+    if (best_cost < 0.0 || cost <= best_cost) { best_cost = cost; best = J; }
+  }
+  return best;
+}
 
 template <int RC>
 int launch_corrector_fluxes() {
@@ -186,16 +209,16 @@ int launch_corrector_fluxes() {
   }
   {
     Box fb = make_box(-1, n0, 0, n1, -1, n2);
-    int J = (n1 + 1 >= 2 * MHD_MARCH_J) ? MHD_MARCH_J : ((n1 + 1 >= 16) ? 8 : 4);
     long long nt = (long long)(n0 + 2) * (n2 + 2);
+    const int J = march_chunk(n1 + 1, grid1(nt, 128).x, 2);
     dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
     k_flux_march<1, RC, false><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<1>");
   }
   {
     Box fb = make_box(-1, n0, -1, n1, 0, n2);
-    int J = (n2 + 1 >= 2 * MHD_MARCH_J) ? MHD_MARCH_J : ((n2 + 1 >= 16) ? 8 : 4);
     long long nt = (long long)(n0 + 2) * (n1 + 2);
+    const int J = march_chunk(n2 + 1, grid1(nt, 128).x, 3);
     dim3 grid(grid1(nt, 128).x, (n2 + 1 + J - 1) / J);
     k_flux_march<2, RC, true><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<2>+update");
