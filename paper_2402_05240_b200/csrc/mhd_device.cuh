@@ -62,6 +62,16 @@ __device__ __forceinline__ double xor_sign(double x, int signbit) {
 // Eq. 12: it is >= 0 analytically; 2^-1000 keeps the seed instruction of the root off 0)
 __device__ __forceinline__ double floor_tiny(double x) { return (hi32(x) < 0x00100000) ? 0x1p-1000 : x; }
 
+// minimum / maximum of two numbers by one compare and one select.  fmin() / fmax() also order NaNs
+// (a predicate pair, two moves, a quiet-bit LOP3 and two selects per call on sm_100a: 7 instructions);
+// their operands here are magnitudes of finite numbers, where both give the same bits.
+__device__ __forceinline__ double min_(double a, double b) { return (a < b) ? a : b; }
+__device__ __forceinline__ double max_(double a, double b) { return (a > b) ? a : b; }
+// the operand of smaller / larger magnitude, sign and all: |x| is free as an operand modifier of the
+// compare but costs an instruction as a value, and every use below ends in copysign() or fabs()
+__device__ __forceinline__ double amin_(double a, double b) { return (fabs(a) < fabs(b)) ? a : b; }
+__device__ __forceinline__ double amax_(double a, double b) { return (fabs(a) > fabs(b)) ? a : b; }
+
 struct HlldSide {
   double rho, u, v, w, P, by, bz;
   double hb2, pT;   // B^2 / 2, total pressure
@@ -418,7 +428,8 @@ __device__ __forceinline__ double sgn3(double x) { return (x > 0.0) ? 1.0 : ((x 
 // "D_f and the cell curvatures share a sign" is tested with products (a fp64 multiply and a compare
 // each, instead of three-way sign extraction), and sgn * min(C|D_a|, C|D_b|, |D_f|) is formed as
 // copysign(min(C min(|D_a|, |D_b|), |D_f|), D_f): multiplication by C = 1.25 is monotone, so the
-// value is bit for bit the oracle's.
+// value is bit for bit the oracle's.  The minima pick the operand of smaller magnitude with its sign
+// (amin_), which copysign() replaces at the end.
 __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, double qd) {
   const double C = 1.25;
   double qf = (7.0 / 12.0) * (qb + qc) - (1.0 / 12.0) * (qa + qd);
@@ -428,7 +439,7 @@ __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, doub
     double Dj1 = qb - 2.0 * qc + qd;
     double Dlim = 0.0;
     if (Df * Dj > 0.0 && Df * Dj1 > 0.0)
-      Dlim = copysign(fmin(C * fmin(fabs(Dj), fabs(Dj1)), fabs(Df)), Df);
+      Dlim = copysign(amin_(C * amin_(Dj, Dj1), Df), Df);
     qf = 0.5 * (qb + qc) - Dlim * (1.0 / 6.0);
   }
   return qf;
@@ -441,7 +452,7 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
   double qp = ppm_face(q1, q2, q3, q4);
   double qi = q2;
   // reading R7: differences that are zero to round-off count as zero in the extremum test
-  double tau = 1e-12 * fmax(fabs(q1), fmax(fabs(q2), fabs(q3)));
+  double tau = 1e-12 * fabs(amax_(q1, amax_(q2, q3)));
   double dm = qi - qm, dp = qp - qi, e3 = q3 - qi, e1 = qi - q1;
   dm = (fabs(dm) <= tau) ? 0.0 : dm;
   dp = (fabs(dp) <= tau) ? 0.0 : dp;
@@ -454,8 +465,8 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
     double Dp1 = q2 - 2.0 * q3 + q4;
     double Dlim = 0.0, r = 0.0;
     if (Df * Dm1 > 0.0 && Df * D0 > 0.0 && Df * Dp1 > 0.0)
-      Dlim = copysign(fmin(C * fmin(fabs(Dm1), fmin(fabs(D0), fabs(Dp1))), fabs(Df)), Df);
-    if (fabs(Df) > fmax(tau, 1e-290)) r = Dlim * rcp(Df);  // (the floor keeps rcp off denormals)
+      Dlim = copysign(amin_(C * amin_(Dm1, amin_(D0, Dp1)), Df), Df);
+    if (fabs(Df) > max_(tau, 1e-290)) r = Dlim * rcp(Df);  // (the floor keeps rcp off denormals)
     if (r <= 1.0 - 1e-12) { qm = qi - r * dm; qp = qi + r * dp; }
   } else {
     if (fabs(dm) >= 2.0 * fabs(dp)) qm = qi - 2.0 * dp;

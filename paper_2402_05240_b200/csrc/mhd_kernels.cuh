@@ -122,7 +122,7 @@ struct Scalars {
 
 __device__ __forceinline__ double warp_max(double v) {
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  for (int o = 16; o > 0; o >>= 1) v = max_(v, __shfl_xor_sync(0xffffffffu, v, o));
   return v;
 }
 
@@ -132,7 +132,7 @@ __device__ __forceinline__ double cell_rate(const Geo &g, const Prim &p, int &ba
 #pragma unroll
   for (int a = 0; a < 3; a++) {
     double cf = sqrt_(fast_speed_sq(g.gamma, p.ir, p.P, p.B[a], p.B[(a + 1) % 3], p.B[(a + 2) % 3]));
-    r = fmax(r, (fabs(p.v[a]) + cf) * g.id[a]);
+    r = max_(r, (fabs(p.v[a]) + cf) * g.id[a]);
   }
   bad |= !isfinite(r) || !(r > 0.0);
   return r;
