@@ -430,6 +430,10 @@ __device__ __forceinline__ double sgn3(double x) { return (x > 0.0) ? 1.0 : ((x 
 // copysign(min(C min(|D_a|, |D_b|), |D_f|), D_f): multiplication by C = 1.25 is monotone, so the
 // value is bit for bit the oracle's.  The minima pick the operand of smaller magnitude with its sign
 // (amin_), which copysign() replaces at the end.
+#ifndef MHD_PPM_BRANCHY
+#define MHD_PPM_BRANCHY 0
+#endif
+#if MHD_PPM_BRANCHY
 __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, double qd) {
   const double C = 1.25;
   double qf = (7.0 / 12.0) * (qb + qc) - (1.0 / 12.0) * (qa + qd);
@@ -474,6 +478,65 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
   }
   qlo = qm; qhi = qp;
 }
+
+#else
+// Branch-free: every candidate value is formed and the tests select among them.  The seven
+// characteristic fields of a cell are then one basic block, whose independent dependency chains the
+// instruction scheduler interleaves (with a branch per test each field was a chain of its own: 2.3-2.5
+// warps waiting on a fixed-latency result per issued instruction, 0.3 on a branch, 0.4-0.6 on instruction
+// fetch); the curvatures D shared by the two faces and by the extremum test are formed once.
+// c ? a : b as one select the compiler cannot turn back into a branch around the evaluation of a
+__device__ __forceinline__ double select_(bool c, double a, double b) {
+  double r;
+  asm("{\n.reg .pred p;\nsetp.ne.s32 p, %3, 0;\nselp.f64 %0, %1, %2, p;\n}" : "=d"(r) : "d"(a), "d"(b), "r"((int)c));
+  return r;
+}
+
+__device__ __forceinline__ double ppm_face(double qa, double qb, double qc, double qd) {
+  const double C = 1.25;
+  const double sbc = qb + qc;
+  const double qf = (7.0 / 12.0) * sbc - (1.0 / 12.0) * (qa + qd);
+  const double Df = 3.0 * (qb - 2.0 * qf + qc);
+  const double Dj = qa - 2.0 * qb + qc;
+  const double Dj1 = qb - 2.0 * qc + qd;
+  const bool same = (Df * Dj > 0.0) && (Df * Dj1 > 0.0);
+  const double Dlim = select_(same, copysign(amin_(C * amin_(Dj, Dj1), Df), Df), 0.0);
+  const double qlim = 0.5 * sbc - Dlim * (1.0 / 6.0);
+  return ((qf - qb) * (qc - qf) < 0.0) ? qlim : qf;
+}
+
+__device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, double q3, double q4,
+                                           double &qlo, double &qhi) {
+  const double C = 1.25;
+  const double qm = ppm_face(q0, q1, q2, q3);
+  const double qp = ppm_face(q1, q2, q3, q4);
+  const double qi = q2;
+  // reading R7: differences that are zero to round-off count as zero in the extremum test
+  const double tau = 1e-12 * fabs(amax_(q1, amax_(q2, q3)));
+  double dm = qi - qm, dp = qp - qi, e3 = q3 - qi, e1 = qi - q1;
+  dm = (fabs(dm) <= tau) ? 0.0 : dm;
+  dp = (fabs(dp) <= tau) ? 0.0 : dp;
+  e3 = (fabs(e3) <= tau) ? 0.0 : e3;
+  e1 = (fabs(e1) <= tau) ? 0.0 : e1;
+  const bool extremum = (dm * dp <= 0.0) || (e3 * e1 <= 0.0);
+  // at an extremum: the parabola's curvature limited against the cell curvatures
+  const double Df = 6.0 * (qm - 2.0 * qi + qp);
+  const double Dm1 = q0 - 2.0 * q1 + q2;
+  const double D0 = q1 - 2.0 * q2 + q3;
+  const double Dp1 = q2 - 2.0 * q3 + q4;
+  const bool same = (Df * Dm1 > 0.0) && (Df * D0 > 0.0) && (Df * Dp1 > 0.0);
+  const double Dlim = select_(same, copysign(amin_(C * amin_(Dm1, amin_(D0, Dp1)), Df), Df), 0.0);
+  const bool big = fabs(Df) > max_(tau, 1e-290);          // (the floor keeps rcp off denormals)
+  const double r = big ? Dlim * rcp(big ? Df : 1.0) : 0.0;
+  const bool shrink = r <= 1.0 - 1e-12;
+  const double qmE = shrink ? qi - r * dm : qm, qpE = shrink ? qi + r * dp : qp;
+  // elsewhere: no overshoot of the parabola inside the cell
+  const double qmM = (fabs(dm) >= 2.0 * fabs(dp)) ? qi - 2.0 * dp : qm;
+  const double qpM = (fabs(dp) >= 2.0 * fabs(dm)) ? qi + 2.0 * dm : qp;
+  qlo = extremum ? qmE : qmM;
+  qhi = extremum ? qpE : qpM;
+}
+#endif
 
 // Wm2..Wp2 = W_{i-2..i+2}; bx0 = cell-centred normal field of cell i
 __device__ __forceinline__ void ppmc(double gamma, const W7 &Wm2, const W7 &Wm1, const W7 &W0,
