@@ -173,8 +173,8 @@ Box make_box(int l0, int h0, int l1, int h1, int l2, int h2) {
 #define MHD_MARCH_J 32
 #endif
 
-int march_chunk(int nfaces, long long blocks_per_chunk, int extra) {
-  const double slots = (double)C.num_sms * MHD_MINB_FM;
+int march_chunk(int nfaces, long long blocks_per_chunk, int extra, int blocks_per_sm) {
+  const double slots = (double)C.num_sms * blocks_per_sm;
   const int n32 = (nfaces + MHD_MARCH_J - 1) / MHD_MARCH_J;
   if ((double)(blocks_per_chunk * n32) > 6.0 * slots) {   // many waves: even chunks of about MHD_MARCH_J
     const int nch = (nfaces + MHD_MARCH_J / 2) / MHD_MARCH_J;
@@ -210,7 +210,7 @@ int launch_corrector_fluxes() {
   {
     Box fb = make_box(-1, n0, 0, n1, -1, n2);
     long long nt = (long long)(n0 + 2) * (n2 + 2);
-    const int J = march_chunk(n1 + 1, grid1(nt, 128).x, 2);
+    const int J = march_chunk(n1 + 1, grid1(nt, 128).x, 2, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM : MHD_MINB_FM);
     dim3 grid(grid1(nt, 128).x, (n1 + 1 + J - 1) / J);
     k_flux_march<1, RC, false><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<1>");
@@ -218,7 +218,7 @@ int launch_corrector_fluxes() {
   {
     Box fb = make_box(-1, n0, -1, n1, 0, n2);
     long long nt = (long long)(n0 + 2) * (n1 + 2);
-    const int J = march_chunk(n2 + 1, grid1(nt, 128).x, 3);
+    const int J = march_chunk(n2 + 1, grid1(nt, 128).x, 3, recon_radius(RC) == 2 ? MHD_MINB_FMZ_PPM : MHD_MINB_FMZ);
     dim3 grid(grid1(nt, 128).x, (n2 + 1 + J - 1) / J);
     k_flux_march<2, RC, true><<<grid, 128, wsm, C.stream>>>(C.Uh, C.F, g, fb, J, C.U, C.sc);
     LAUNCH_CHECK("k_flux_march<2>+update");

@@ -274,6 +274,10 @@ __device__ __forceinline__ void pcm_face(double (*st)[MHD_PRED_T], const State8 
 #ifndef MHD_MINB_FX_PPM
 #define MHD_MINB_FX_PPM 4
 #endif
+// the 5-cell z sweep with the update wants 212 registers (2.08 -> 2.00 ms at 256^3 against 3 blocks of 168)
+#ifndef MHD_MINB_FMZ_PPM
+#define MHD_MINB_FMZ_PPM 2
+#endif
 __global__ void __launch_bounds__(MHD_PRED_T, MHD_MINB_PRED) k_predictor_flux(State8 U, Flux21 F, Edge3 Er, Geo g, Box box) {
   __shared__ double st[33][MHD_PRED_T];
   const int lx = box.hi[0] - box.lo[0] + 1, ly = box.hi[1] - box.lo[1] + 1;
@@ -533,7 +537,7 @@ __global__ void __launch_bounds__(128, RC == 2 ? MHD_MINB_FX_PPM : MHD_MINB_FX) 
 // do, for the CT kernel), and the full update that follows only has the face field left to do.
 // A chunk then also solves face f1+1 (its last cell needs it; 1/J more Riemann solves).
 template <int A, int RC, bool UPDATE>
-__global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? MHD_MINB_FM_PPM : (UPDATE ? MHD_MINB_FMZ : MHD_MINB_FM)) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
+__global__ void __launch_bounds__(128, recon_radius(RC) == 2 ? (UPDATE ? MHD_MINB_FMZ_PPM : MHD_MINB_FM_PPM) : (UPDATE ? MHD_MINB_FMZ : MHD_MINB_FM)) k_flux_march(State8 Uh, Flux21 F, Geo g, Box fb, int J,
                                                                   State8 U, const Scalars *sc) {
   static_assert(!UPDATE || A == 2, "the fused hydro update rides on the z sweep");
   constexpr int R = recon_radius(RC);
