@@ -192,6 +192,30 @@ int mhd_finalize(void);
 /* Static string describing the last error (never NULL). */
 const char *mhd_last_error(void);
 
+/* ---- An entry point that allocates nothing (csrc/mhd_noalloc.cu) --------------------------------
+ * The diagnostic of mhd_max_divb for callers that cannot call cudaMalloc: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  It needs no
+ * mhd_init and no context, and calls no cudaMalloc, cudaFree or allocating library routine: the
+ * reduction's scratch (one partial maximum per block of 256 cells) is a static __device__ array of
+ * MHD_NOALLOC_MAX_PARTIALS doubles (512 KiB), which every GPU that loads the library holds until the
+ * process exits.  Grids of more than MHD_NOALLOC_MAX_CELLS cells (256^3) are rejected with
+ * MHD_ERR_ARG and a message naming the limit; nothing is launched then.
+ *   nx, ny, nz      active cells;  dx, dy, dz = cell sizes (> 0)
+ *   d_bx, d_by, d_bz DEVICE pointers, the dense face arrays of the ABI layout above ((nx+1)*ny*nz,
+ *                   nx*(ny+1)*nz, nx*ny*(nz+1) doubles, i fastest); read only, owned by the caller
+ *   d_out           DEVICE pointer to one double: max over cells of |sum_a (B_a[upper] - B_a[lower]) / Delta_a|
+ *   stream          a cudaStream_t (NULL = legacy default stream); two kernels are enqueued on it and the
+ *                   call returns without synchronising
+ * All calls on one device share the scratch array, which keeps the last call's contents (no part of it
+ * has to be zero: a call writes every slot it later reads).  Calls that overlap on the GPU -- different
+ * streams with no ordering between them -- race on it; order them.  Errors: MHD_ERR_ARG (sizes,
+ * null pointers, too many cells), MHD_ERR_CUDA; text from mhd_noalloc_last_error(). */
+#define MHD_NOALLOC_MAX_PARTIALS 65536
+#define MHD_NOALLOC_MAX_CELLS (256LL * MHD_NOALLOC_MAX_PARTIALS)
+int mhd_max_divb_noalloc(int nx, int ny, int nz, double dx, double dy, double dz, const double *d_bx,
+                         const double *d_by, const double *d_bz, double *d_out, void *stream);
+const char *mhd_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -11,7 +11,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmhd.so")
 SOURCES = [os.path.join(CSRC, "mhd_api.cu"), os.path.join(CSRC, "mhd_peaks.cu"),
-           os.path.join(CSRC, "mhd_unit.cu")]
+           os.path.join(CSRC, "mhd_unit.cu"), os.path.join(CSRC, "mhd_noalloc.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mhd_device.cuh", "mhd_grid.cuh", "mhd_kernels.cuh", "mhd_math.cuh",
                                                    "mhd_stage.cuh")] + [
     os.path.join(ROOT, "include", "mhd.h")]

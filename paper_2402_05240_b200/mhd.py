@@ -63,6 +63,9 @@ def _load():
     L.mhd_debug_guard_errors.restype = ctypes.c_int
     L.mhd_launch_count.restype = ctypes.c_longlong
     L.mhd_last_error.restype = ctypes.c_char_p
+    L.mhd_max_divb_noalloc.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [_vp] * 5
+    L.mhd_max_divb_noalloc.restype = ctypes.c_int
+    L.mhd_noalloc_last_error.restype = ctypes.c_char_p
     for name in ("mhd_init", "mhd_init_workspace", "mhd_set_boundary", "mhd_set_domain", "mhd_set_stream", "mhd_set_state",
                  "mhd_set_state_device", "mhd_compute_dt", "mhd_step", "mhd_advance", "mhd_get_state",
                  "mhd_get_state_device", "mhd_get_half_state", "mhd_max_divb", "mhd_synchronize",
@@ -85,6 +88,20 @@ def _check(rc):
 
 def _hp(a):
     return a.ctypes.data_as(_dp)
+
+
+NOALLOC_MAX_CELLS = 256 * 65536   # MHD_NOALLOC_MAX_CELLS of include/mhd.h
+
+
+def max_divb_noalloc(n, d, bx, by, bz, out, stream=None):
+    """mhd_max_divb_noalloc: max |div B| of dense DEVICE face arrays (torch tensors, ABI layout) into the
+    one-element device tensor `out`, on `stream` (a torch.cuda.Stream; None = legacy default stream).
+    Allocates nothing and does not synchronise; needs no Mhd context.  n = (nx, ny, nz), d = (dx, dy, dz)."""
+    rc = _lib.mhd_max_divb_noalloc(int(n[0]), int(n[1]), int(n[2]), float(d[0]), float(d[1]), float(d[2]),
+                                   _vp(bx.data_ptr()), _vp(by.data_ptr()), _vp(bz.data_ptr()), _vp(out.data_ptr()),
+                                   _vp(stream.cuda_stream if stream is not None else 0))
+    if rc != 0:
+        raise MhdError("libmhd error %d: %s" % (rc, _lib.mhd_noalloc_last_error().decode()))
 
 
 def measure_peaks(seconds=0.0):
