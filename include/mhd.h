@@ -145,6 +145,13 @@ int mhd_max_divb(double *out);
  * the per-kernel roofline; the state advances exactly as with mhd_step. */
 int mhd_step_profile(double dt, int max_entries, double *ms, const char **names, int *n_entries);
 
+/* The same for n_steps (1..4096) consecutive steps of mhd_advance (each with its own dt from the CFL
+ * reduction), enqueued back to back without synchronisation in between: ms[i] is the
+ * duration of launch i of a step averaged over the steps (launch 0 is the dt kernel), i.e. the
+ * kernels' durations in the steady state of a long run.  Always the kernel-per-stage path (no CUDA
+ * graph, no cooperative small-grid kernel).  Synchronises at the end.  Used by bench.py for the roofline. */
+int mhd_advance_profile(int n_steps, double cfl, int max_entries, double *ms, const char **names, int *n_entries);
+
 /* Roofline denominators measured on the current device (not part of the time step): the fp64
  * FMA-pipe peak in TFLOP/s from a kernel of independent DFMA chains (8 per thread, 2048 threads
  * per SM; burst = best of 5 launches if seconds <= 0.5, else the mean over the second half of 40

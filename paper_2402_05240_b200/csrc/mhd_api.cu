@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <vector>
 #include <cuda_runtime.h>
 
 #include "../../include/mhd.h"
@@ -50,8 +51,9 @@ struct Context {
   int parity = 0;  // flips with every step (which set of face arrays holds B^n)
   // per-launch event timing (mhd_step_profile)
   int prof_n = -1;  // -1 = off, else number of launches recorded so far
-  cudaEvent_t prof_ev[kMaxProf + 1];
-  const char *prof_name[kMaxProf];
+  int prof_cap = 0; // launches the two arrays below can take (they belong to the profiling call in progress)
+  cudaEvent_t *prof_ev = nullptr;
+  const char **prof_name = nullptr;
 };
 
 Context C;
@@ -79,7 +81,7 @@ int cuda_fail(cudaError_t e, const char *where) {
     C.launches++;                                                   \
     cudaError_t e_ = cudaGetLastError();                            \
     if (e_ != cudaSuccess) return cuda_fail(e_, name);              \
-    if (C.prof_n >= 0 && C.prof_n < kMaxProf) {                     \
+    if (C.prof_n >= 0 && C.prof_n < C.prof_cap) {                   \
       C.prof_name[C.prof_n] = name;                                 \
       cudaEventRecord(C.prof_ev[++C.prof_n], C.stream);             \
     }                                                               \
@@ -758,28 +760,74 @@ int mhd_max_divb(double *out) {
   return MHD_OK;
 }
 
+// n_steps steps with a CUDA event after every launch, all enqueued back to back (no synchronisation
+// until the last one), then the duration of launch i of a step averaged over the steps.
+// cfl > 0: every step takes its own dt from the CFL reduction, as mhd_advance does; else the given dt.
+int profiled_steps(int n_steps, double dt, double cfl, int max_entries, double *ms, const char **names, int *n_entries) {
+  const int cap = kMaxProf * n_steps;
+  std::vector<cudaEvent_t> ev((size_t)cap + 1, nullptr);
+  std::vector<const char *> nm((size_t)cap, nullptr);
+  int rc = MHD_OK;
+  for (auto &e : ev)
+    if (!rc && cudaEventCreate(&e) != cudaSuccess) rc = fail(MHD_ERR_CUDA, "cudaEventCreate failed");
+  auto enqueue = [&]() -> int {
+    if (cfl > 0.0) {
+      int r = ensure_rate();
+      if (r) return r;
+    } else {
+      k_set_dt<<<1, 1, 0, C.stream>>>(C.sc, dt);
+      LAUNCH_CHECK("k_set_dt");
+    }
+    C.prof_ev = ev.data(); C.prof_name = nm.data(); C.prof_cap = cap;
+    C.prof_n = 0;
+    cudaEventRecord(ev[0], C.stream);
+    for (int s = 0; s < n_steps; s++) {
+      if (cfl > 0.0) {
+        k_finish_dt<<<1, 1, 0, C.stream>>>(C.sc, cfl);
+        LAUNCH_CHECK("k_finish_dt");
+      }
+      int r = step_kernels();
+      if (r) return r;
+    }
+    return MHD_OK;
+  };
+  if (!rc) rc = enqueue();
+  const int n = C.prof_n;
+  C.prof_n = -1; C.prof_cap = 0; C.prof_ev = nullptr; C.prof_name = nullptr;
+  cudaError_t e = cudaStreamSynchronize(C.stream);
+  if (!rc && e != cudaSuccess) rc = cuda_fail(e, "cudaStreamSynchronize");
+  *n_entries = 0;
+  if (!rc && n > 0 && n % n_steps == 0) {
+    const int per = n / n_steps;
+    for (int i = 0; i < per && i < max_entries; i++) {
+      double sum = 0.0;
+      for (int s = 0; s < n_steps; s++) {
+        float t = 0.f;
+        cudaEventElapsedTime(&t, ev[(size_t)s * per + i], ev[(size_t)s * per + i + 1]);
+        sum += t;
+      }
+      ms[i] = sum / n_steps; names[i] = nm[i]; *n_entries = i + 1;
+    }
+  } else if (!rc) {
+    rc = fail(MHD_ERR_CUDA, "profiled steps recorded an unexpected number of launches");
+  }
+  for (auto &x : ev)
+    if (x) cudaEventDestroy(x);
+  return rc;
+}
+
 int mhd_step_profile(double dt, int max_entries, double *ms, const char **names, int *n_entries) {
   if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
   if (!(dt > 0.0) || !ms || !names || !n_entries || max_entries < 1)
     return fail(MHD_ERR_ARG, "mhd_step_profile: bad argument");
-  for (int i = 0; i <= kMaxProf; i++) CU(cudaEventCreate(&C.prof_ev[i]));
-  k_set_dt<<<1, 1, 0, C.stream>>>(C.sc, dt);
-  LAUNCH_CHECK("k_set_dt");
-  C.prof_n = 0;
-  cudaEventRecord(C.prof_ev[0], C.stream);
-  int rc = step_kernels();
-  int n = C.prof_n;
-  C.prof_n = -1;
-  cudaError_t e = cudaStreamSynchronize(C.stream);
-  if (!rc && e != cudaSuccess) rc = cuda_fail(e, "cudaStreamSynchronize");
-  *n_entries = 0;
-  for (int i = 0; i < n && !rc; i++) {
-    float t = 0.f;
-    cudaEventElapsedTime(&t, C.prof_ev[i], C.prof_ev[i + 1]);
-    if (i < max_entries) { ms[i] = t; names[i] = C.prof_name[i]; *n_entries = i + 1; }
-  }
-  for (int i = 0; i <= kMaxProf; i++) cudaEventDestroy(C.prof_ev[i]);
-  return rc;
+  return profiled_steps(1, dt, 0.0, max_entries, ms, names, n_entries);
+}
+
+int mhd_advance_profile(int n_steps, double cfl, int max_entries, double *ms, const char **names, int *n_entries) {
+  if (!C.inited) return fail(MHD_ERR_NOT_INIT, "not initialised");
+  if (n_steps < 1 || n_steps > 4096 || !(cfl > 0.0) || !ms || !names || !n_entries || max_entries < 1)
+    return fail(MHD_ERR_ARG, "mhd_advance_profile: bad argument");
+  return profiled_steps(n_steps, 0.0, cfl, max_entries, ms, names, n_entries);
 }
 
 int mhd_debug_guard_errors(long long *n_bad) {

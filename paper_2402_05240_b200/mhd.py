@@ -55,6 +55,9 @@ def _load():
     L.mhd_step_profile.argtypes = [ctypes.c_double, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_char_p),
                                    ctypes.POINTER(ctypes.c_int)]
     L.mhd_step_profile.restype = ctypes.c_int
+    L.mhd_advance_profile.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_char_p),
+                                      ctypes.POINTER(ctypes.c_int)]
+    L.mhd_advance_profile.restype = ctypes.c_int
     L.mhd_unit_hlld.argtypes = [ctypes.c_int, ctypes.c_double, _dp, _dp, _dp, _dp]
     L.mhd_unit_reconstruct.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_int, _dp, _dp, _dp, _dp]
     L.mhd_unit_ct_edge.argtypes = [ctypes.c_int, _dp, _dp]
@@ -249,6 +252,14 @@ class Mhd:
         names = (ctypes.c_char_p * max_entries)()
         n = ctypes.c_int()
         _check(_lib.mhd_step_profile(float(dt), max_entries, ms, names, ctypes.byref(n)))
+        return [(names[i].decode(), ms[i]) for i in range(n.value)]
+
+    def advance_profile(self, n_steps, cfl, max_entries=32):
+        """n_steps instrumented steps of advance(), back to back: list of (kernel name, mean milliseconds)."""
+        ms = (ctypes.c_double * max_entries)()
+        names = (ctypes.c_char_p * max_entries)()
+        n = ctypes.c_int()
+        _check(_lib.mhd_advance_profile(int(n_steps), float(cfl), max_entries, ms, names, ctypes.byref(n)))
         return [(names[i].decode(), ms[i]) for i in range(n.value)]
 
     def get_flux(self, axis, comp):
