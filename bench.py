@@ -384,7 +384,6 @@ def run_b200(args):
         barrier()
         ms = e0.elapsed_time(e1)
         launches = g.launch_count() - l0
-        clocks = sampler.stop() if rank == 0 else None
         value, ms = job_value(ms, nc, args.steps, world)
         # ---- per-kernel live timing (CUDA events on the library stream) ----------------
         # Directly behind the timed region, the same K steps enqueued back to back in the same way with an
@@ -401,6 +400,7 @@ def run_b200(args):
             e1.record(stream)
             torch.cuda.synchronize()
             reps.append(job_value(e0.elapsed_time(e1), nc, args.steps, world)[1] / args.steps)
+        clocks = sampler.stop() if rank == 0 else None   # sampled over the timed region, the profiled one and the repeats
 
         bad_state = False
         try:
