@@ -317,6 +317,35 @@ def test_advance_matches_stepwise_and_device_io(mhd, monkeypatch):
     g.close()
 
 
+def test_advance_profile_is_bitwise_advance_and_names_its_kernels(mhd, monkeypatch):
+    """mhd_advance_profile (bench.py's per-kernel times) runs the steps of mhd_advance with an event after
+    every launch: the state after K profiled steps is bit for bit that of K plain steps, a step is the dt
+    kernel plus six stage kernels, every duration is positive, and a following plain call carries on."""
+    monkeypatch.setenv("MHD_SMALL", "0")
+    p = inputs.random_smooth(n=(45, 33, 21), seed=5, recon=1)
+    ref = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc)
+    ref.set_state(p.state)
+    for _ in range(5):
+        ref.step(ref.compute_dt(0.4))
+    want = ref.get_state()
+    ref.close()
+    g = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc)
+    g.set_state(p.state)
+    prof = g.advance_profile(3, 0.4)
+    assert [name for name, _ in prof] == ["k_finish_dt", "k_predictor_stage", "k_flux_x", "k_flux_march<1>",
+                                          "k_flux_march<2>+update", "k_ct(corrector)", "k_update(B)+cfl"]
+    assert all(t > 0.0 for _, t in prof)
+    g.advance(2, 0.4)
+    got = g.get_state()
+    for f in FIELDS:
+        assert np.array_equal(got[f], want[f]), f
+    one = g.step_profile(g.compute_dt(0.4))              # the one-step variant still returns the six stage kernels
+    assert [name for name, _ in one] == [name for name, _ in prof][1:]
+    with pytest.raises(mhd.MhdError):
+        g.advance_profile(0, 0.4)
+    g.close()
+
+
 @pytest.mark.parametrize("recon,bc", [(1, (0, 0, 0)), (2, (1, 0, 0))])
 def test_advance_graph_path_is_bitwise_the_stepwise_path(mhd, recon, bc, monkeypatch):
     """On a non-default stream and a small grid mhd_advance replays a CUDA graph of two steps; an odd
