@@ -179,8 +179,8 @@ int march_chunk(int nfaces, long long blocks_per_chunk, int extra, int blocks_pe
   const double slots = (double)C.num_sms * blocks_per_sm;
   const int n32 = (nfaces + MHD_MARCH_J - 1) / MHD_MARCH_J;
   if ((double)(blocks_per_chunk * n32) > 6.0 * slots) {   // many waves: even chunks of about MHD_MARCH_J
-    const int nch = (nfaces + MHD_MARCH_J / 2) / MHD_MARCH_J;
-    return (nfaces + nch - 1) / nch;
+    const int nch = (nfaces + MHD_MARCH_J / 2) / MHD_MARCH_J;   // (0 for a thin slab: one chunk)
+    return nch < 1 ? nfaces : (nfaces + nch - 1) / nch;
   }
   int best = nfaces;
   double best_cost = -1.0;

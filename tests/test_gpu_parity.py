@@ -317,6 +317,22 @@ def test_advance_matches_stepwise_and_device_io(mhd, monkeypatch):
     g.close()
 
 
+@pytest.mark.parametrize("n", [(600, 3, 600), (600, 600, 3), (3, 700, 520)])
+def test_thin_slabs_with_many_blocks(mhd, n):
+    """Grids with a handful of cells along one sweep axis and thousands of blocks across it (the marching
+    sweeps then take one chunk per column; a chunk count of zero once divided by zero here): one PLMC
+    step against the oracle."""
+    p = inputs.random_smooth(n=n, seed=9, recon=1)
+    o, g = make_pair(mhd, p)
+    dt = o.compute_dt(p.cfl)
+    assert abs(g.compute_dt(p.cfl) - dt) <= 1e-13 * dt
+    o.step(dt); g.step(dt)
+    out = g.get_state()
+    assert_close(out, o.get_state(), TOL_STEP, "thin slab %s" % (n,))
+    assert divb_normalised(out, p.n) <= TOL_DIVB
+    o.close(); g.close()
+
+
 def test_advance_profile_is_bitwise_advance_and_names_its_kernels(mhd, monkeypatch):
     """mhd_advance_profile (bench.py's per-kernel times) runs the steps of mhd_advance with an event after
     every launch: the state after K profiled steps is bit for bit that of K plain steps, a step is the dt
