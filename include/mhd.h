@@ -69,7 +69,7 @@ int mhd_init(int nx, int ny, int nz, double gamma, int recon);
 int mhd_init_workspace(int nx, int ny, int nz, double gamma, int recon, void *workspace,
                        size_t workspace_bytes);
 
-/* axis 0/1/2 = x/y/z; kind MHD_BC_*.  Takes effect at the next ghost fill (the next
+/* axis 0/1/2 = x/y/z; kind MHD_BC_*.  Takes effect at the next boundary update (the next
  * mhd_set_state* or mhd_step). */
 int mhd_set_boundary(int axis, int kind);
 
@@ -96,7 +96,7 @@ int mhd_set_state_device(const double *rho, const double *mx, const double *my,
  * (PAPER.md:317-327).  Synchronous: *dt (HOST pointer) is valid on return. */
 int mhd_compute_dt(double cfl, double *dt);
 
-/* One full VL+CT step of size dt (steps 2-9): ghost fill, PCM+HLLD
+/* One full VL+CT step of size dt (steps 2-9): boundary update, PCM+HLLD
  * predictor fluxes, CT edge fields, half update, high-order reconstruction + HLLD, CT edge
  * fields, full update.  Asynchronous on the library stream. */
 int mhd_step(double dt);
