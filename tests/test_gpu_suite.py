@@ -29,13 +29,17 @@ def pair(mhd, p):
     return o, g
 
 
-def stepwise(mhd, p, n_steps, what, alfven_units=False):
+def stepwise(mhd, p, n_steps, what, alfven_units=False, switch_steps=0, switch_cells=0):
     """n_steps one-step parity cases, each from the oracle's own state.  alfven_units: the field is a
     passive tracer (|B| << sqrt(rho)|v|, field loop): the round-off of the O(1) velocities enters the
-    induction equation at 1e-16 ABSOLUTE, so B is compared in units of max(|B|, |m|/sqrt(rho))."""
+    induction equation at 1e-16 ABSOLUTE, so B is compared in units of max(|B|, |m|/sqrt(rho)).
+    switch_steps / switch_cells: at most that many steps may miss the tolerance, each in at most that
+    many cells per field (a discontinuous limiter switch taken on the other side, DESIGN.md R11);
+    every other step and every other cell is held to TOL_STEP."""
     o, g = pair(mhd, p)
     state = p.state
     worst = 0.0
+    off_steps = []
     for s in range(n_steps):
         g.set_state(state)
         dt = o.compute_dt(p.cfl)
@@ -48,8 +52,15 @@ def stepwise(mhd, p, n_steps, what, alfven_units=False):
             vs = max(np.abs(state[m]).max() for m in ("mx", "my", "mz")) / np.sqrt(state["rho"].max())
             for f in ("bx", "by", "bz"):
                 rd[f] = np.abs(out[f] - state[f]).max() / max(np.abs(state[f]).max(), vs)
-        assert max(rd.values()) <= TOL_STEP, "%s step %d: %s" % (what, s + 1, rd)
         assert divb_normalised(out, p.n, p.domain) <= TOL_DIVB
+        if max(rd.values()) > TOL_STEP and switch_steps:
+            cells = max(int((np.abs(out[f] - state[f]) > TOL_STEP * max(np.abs(state[f]).max(), 1e-300)).sum())
+                        for f in FIELDS)
+            assert cells <= switch_cells, "%s step %d: %d cells off, %s" % (what, s + 1, cells, rd)
+            off_steps.append(s + 1)
+            assert len(off_steps) <= switch_steps, "%s: steps off %s" % (what, off_steps)
+            continue
+        assert max(rd.values()) <= TOL_STEP, "%s step %d: %s" % (what, s + 1, rd)
         worst = max(worst, max(rd.values()))
     o.close(); g.close()
     return worst
@@ -127,9 +138,14 @@ def test_blast_in_the_papers_box(mhd, recon):
     """PAPER.md:455-465 at 24 x 36 x 24 in the 1 x 1.5 x 1 box: 10 one-step parity cases; free run of
     the PLMC case keeps the z-mirror and point symmetries at round-off (R11 for PPMC)."""
     p = inputs.blast_paper(24, recon=recon)
-    # PPMC: from the third step on the mirror-symmetric flat tops of this problem sit on the PPM
-    # extremum switch (DESIGN.md R11) and no two implementations stay together; two steps are exact.
-    stepwise(mhd, p, 10 if recon == 1 else 2, "paper blast recon %d" % recon)
+    # PPMC: the mirror-symmetric flat tops of this problem sit on the PPM extremum switch (DESIGN.md R11),
+    # where a difference in the last bit of an amplitude selects another parabola: seen in one of the ten
+    # steps (the fourth: 66 of 20,736 cells per field, up to 3e-5).  At most one such step and at most
+    # 132 such cells are let through; the other nine steps agree to 1e-13.
+    if recon == 1:
+        stepwise(mhd, p, 10, "paper blast recon 1")
+    else:
+        stepwise(mhd, p, 10, "paper blast recon 2", switch_steps=1, switch_cells=132)
     g = mhd.Mhd(*p.n, p.gamma, p.recon, p.bc, domain=p.domain)
     g.set_state(p.state)
     for _ in range(12):
