@@ -191,10 +191,10 @@ def test_c2_brio_wu_outflow(mhd):
             d = p.t_end - t
         g.step(d); t += d; n_g += 1
     out, ref = g.get_state(), o.get_state()
-    # the two runs take their own dt (both from Eq. 11); they must agree to round-off growth
-    assert abs(n_g - n_o) <= 1
-    if n_g == n_o:
-        assert_close(out, ref, 1e-8, "C2 final state")
+    # the two runs take their own dt (both from Eq. 11): same number of steps (243), and the final states
+    # agree within north_star's full-run tolerance (seen: 3e-14)
+    assert n_g == n_o
+    assert_close(out, ref, TOL_RUN, "C2 final state")
     # planar invariants (pin T12)
     assert np.all(out["bx"] == 0.75)
     assert np.max(np.abs(out["mz"])) <= 1e-14 and np.max(np.abs(out["bz"])) <= 1e-14
