@@ -28,7 +28,8 @@
  * Parity unpinned (choice among valid variants, no author code or printed
  * numbers to compare against): HLLD wave-speed estimate and degeneracy
  * tolerance (G15), eigenvector normalisation in degenerate states (G16), the
- * PPM variant (G17, O10), outflow boundary treatment (G24).  Each of these is
+ * PPM variant (G17, O10; its constant C is bracketed by a smooth-extremum pin),
+ * outflow boundary treatment (G24).  Each of these is
  * pinned to the mathematics it must satisfy (consistency, exactness on
  * polynomials, L.R = I ...) but not to the authors' code.
  *

@@ -317,6 +317,38 @@ def test_T11_ppm_monotone_and_bounded():
     assert lo == 1.0 and hi == 1.0
 
 
+def _cos_cell_averages(n_cells, j, phase):
+    """Exact cell average of cos(2 pi x + phase) over cell j of n_cells on the unit interval."""
+    a, b = j / n_cells, (j + 1) / n_cells
+    return (np.sin(2 * np.pi * b + phase) - np.sin(2 * np.pi * a + phase)) / (2 * np.pi * (b - a))
+
+
+def test_ppm_limiter_constant_is_bracketed_by_smooth_extrema():
+    """Reading G17 takes the curvature limiter's constant C = 1.25 from the cited PPM (PAPER.md:231);
+    nothing else pinned it (round-1 review: "changing it is not caught").  Its job is to leave smooth
+    extrema alone and to clip under-resolved ones, and a cosine decides which is which: at an extremum
+    the parabola's curvature exceeds the smallest neighbouring cell curvature by a factor that depends
+    only on the resolution and on where the extremum sits in its cell -- 1.165 at 16 cells per wavelength
+    with the extremum at a cell centre, 1.269 with the extremum on a face, 1.309 at 12 cells (centre),
+    <= 1.11 at 24.  So with C = 1.25 the first and the last are reconstructed with the unlimited
+    fourth-order face values of the textbook formula, bit for bit, and the other two are clipped; a
+    constant below 1.165 fails the first assertion, one above 1.269 the second."""
+    def deviation(n_cells, phase):
+        worst = 0.0
+        for j in range(n_cells):
+            q = np.array([_cos_cell_averages(n_cells, j + s, phase) for s in (-2, -1, 0, 1, 2)])
+            lo, hi = orc.ppm_scalar(q)
+            face_lo = 7.0 / 12.0 * (q[1] + q[2]) - 1.0 / 12.0 * (q[0] + q[3])
+            face_hi = 7.0 / 12.0 * (q[2] + q[3]) - 1.0 / 12.0 * (q[1] + q[4])
+            worst = max(worst, abs(lo - face_lo), abs(hi - face_hi))
+        return worst
+    assert deviation(16, -np.pi / 16) <= 2e-16      # extremum at a cell centre, ratio 1.165: untouched
+    assert deviation(24, 0.0) <= 2e-16 and deviation(24, -np.pi / 24) <= 2e-16
+    assert deviation(32, 0.0) <= 2e-16
+    assert deviation(16, 0.0) > 1e-4                # extremum on a face, ratio 1.269: clipped
+    assert deviation(12, -np.pi / 12) > 1e-4        # ratio 1.309: clipped
+
+
 def test_ppmc_constant_and_linear_vector():
     rng = np.random.default_rng(8)
     W0 = rand_state(rng)
