@@ -163,6 +163,32 @@ def hllc_textbook(gamma, WL, WR):
     return flux(WR) + SR * (star(WR, SR) - cons(WR))
 
 
+def test_hlld_outer_speeds_use_both_states_fast_speeds():
+    """Reading G15: S_L = min(u_L, u_R) - max(c_fL, c_fR), S_R = max(u_L, u_R) + max(c_fL, c_fR) (the
+    second of the two estimates Miyoshi & Kusano offer; the paper names none).  The other
+    one, S_L = min(u_L - c_fL, u_R - c_fR), differs exactly where one side is much hotter than the other:
+    here both states move to the right faster than their OWN fast speed (u - c_f = 2.25 and 1.30), so the
+    own-side estimate calls the face supersonic and returns F_L, while the left state is overrun by the
+    right state's fast wave (min u - max c_f = -0.70 < 0) and the estimate of the reading opens the fan.
+    The test fixes which of the two the oracle implements; the mirror image does the same for S_R."""
+    WL = np.array([1.0, 3.0, 0.1, -0.2, 0.3, 0.2, 0.1])
+    WR = np.array([1.0, 5.0, 0.2, 0.1, 8.0, 0.5, -0.3])
+    bx = 0.4
+    cL = orc.fast_speed(G, WL[0], WL[4], bx, WL[5], WL[6])
+    cR = orc.fast_speed(G, WR[0], WR[4], bx, WR[5], WR[6])
+    assert WL[1] - cL > 1.0 and WR[1] - cR > 1.0 and min(WL[1], WR[1]) - max(cL, cR) < -0.5
+    F, FL = orc.hlld(G, WL, WR, bx), orc.phys_flux(G, WL, bx)
+    assert np.max(np.abs(F - FL)) > 1e-2                   # not the supersonic branch
+    assert F[0] < FL[0]                                    # the fan lets mass through more slowly than rho_L u_L
+    # a genuinely supersonic face (cold on both sides) still returns F_L bit for bit
+    WRc = WR.copy(); WRc[4] = 0.3
+    assert np.array_equal(orc.hlld(G, WL, WRc, bx), FL)
+    # mirror image: S_R
+    flip = np.array([1.0, -1.0, -1.0, 1.0, 1.0, -1.0, 1.0])
+    Fm, FRm = orc.hlld(G, WR * flip, WL * flip, -bx), orc.phys_flux(G, WL * flip, -bx)
+    assert np.max(np.abs(Fm - FRm)) > 1e-2
+
+
 def test_T5_hlld_reduces_to_hllc_without_field():
     rng = np.random.default_rng(4)
     for it in range(500):
