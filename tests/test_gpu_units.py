@@ -25,7 +25,7 @@ def ulps(a, b):
 
 
 def test_math_rcp_rsqrt_sqrt_within_two_ulp(mhd):
-    """csrc/mhd_math.cuh (hardware seed + two Newton steps) against IEEE division / sqrt."""
+    """csrc/mhd_math.cuh (hardware seed + one cubically convergent step) against IEEE division / sqrt."""
     rng = np.random.default_rng(11)
     x = 10.0 ** rng.uniform(-30, 30, size=200000)
     x[:5] = [1.0, 2.0, 0.5, 3.0, 1e-200]
@@ -52,6 +52,16 @@ def hlld_cases():
     for vs, bs, n in ((1.0, 1.0, 3000), (4.0, 0.3, 1500), (0.1, 2.0, 1500), (1.0, 0.0, 300)):
         WL.append(rand_states(rng, n, vs, bs)); WR.append(rand_states(rng, n, vs, bs))
         bx.append(rng.normal(size=n) * bs)
+    # a hot state overrunning a cold one, both moving faster than their own fast speed: the regime in which
+    # the two outer-speed estimates of Miyoshi & Kusano differ (reading G15, tests/test_oracle_units.py)
+    n = 1000
+    hot, cold = rand_states(rng, n, 0.3, 0.5), rand_states(rng, n, 0.3, 0.5)
+    hot[:, 4] = rng.uniform(4.0, 20.0, n); cold[:, 4] = rng.uniform(0.05, 0.5, n)
+    drift = rng.uniform(1.5, 6.0, n) * rng.choice([-1.0, 1.0], n)
+    hot[:, 1] += drift; cold[:, 1] += drift
+    swap = rng.uniform(size=n) < 0.5
+    WL.append(np.where(swap[:, None], hot, cold)); WR.append(np.where(swap[:, None], cold, hot))
+    bx.append(rng.normal(size=n) * 0.5)
     WL, WR, bx = np.concatenate(WL), np.concatenate(WR), np.concatenate(bx)
     bx[::7] = 0.0                       # B_x = 0: no double-star region
     WR[5::11] = WL[5::11]               # identical states: F(U,U) = F(U)
