@@ -79,6 +79,22 @@ def test_hlld_all_branches(mhd):
     assert (np.abs(F - ref) / scale).max() <= 1e-12
 
 
+def test_hlld_exactly_degenerate_rotational_discontinuity(mhd):
+    """The state of tests/test_oracle_units.py::test_hlld_degenerate_star_state, (a): gamma = 3/2, every
+    intermediate exact, D = 0.0 -- the 0/0 of the star state -- and its neighbours B_perp = 1e-14 ... 1e-3."""
+    WL = np.array([[1.0, 0.25, 0.5, -0.25, 0.5, 0.0, 0.0]])
+    WR = np.array([[1.0, 0.25, -0.5, 0.75, 0.5, 0.0, 0.0]])
+    F = mhd.unit_hlld(1.5, WL, WR, np.array([2.0]))[0]
+    ref = orc.hlld(1.5, WL[0], WR[0], 2.0)
+    assert np.all(np.isfinite(F)) and np.abs(F - ref).max() <= 1e-15
+    deltas = 10.0 ** np.arange(-14.0, -2.5, 0.5)
+    L = np.repeat(WL, len(deltas), axis=0); R = np.repeat(WR, len(deltas), axis=0)
+    L[:, 5] = deltas; L[:, 6] = -0.5 * deltas; R[:, 5] = 0.3 * deltas; R[:, 6] = deltas
+    Fd = mhd.unit_hlld(1.5, L, R, np.full(len(deltas), 2.0))
+    refd = np.array([orc.hlld(1.5, L[i], R[i], 2.0) for i in range(len(deltas))])
+    assert np.all(np.isfinite(Fd)) and np.abs(Fd - refd).max() <= 1e-12
+
+
 def test_hlld_mass_flux_is_exactly_zero_between_mirror_states(mhd):
     """Reading R6 (Eq. 16 'otherwise' branch): mirror-image states at rest or colliding give an
     exactly zero mass flux on both sides, whatever the round-off of S_M."""

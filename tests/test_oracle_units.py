@@ -189,6 +189,51 @@ def test_hlld_outer_speeds_use_both_states_fast_speeds():
     assert np.max(np.abs(Fm - FRm)) > 1e-2
 
 
+def test_hlld_degenerate_star_state():
+    """Reading G15, second half: where D = rho (S - u)(S - S_M) - B_x^2 vanishes the star state's
+    tangential jump is 0/0 and Miyoshi & Kusano prescribe "no jump" (taken below |D| < 1e-8 p_T*).  That
+    happens for a strong normal field (c_f = c_a), no jump in u and p_T, and B_perp = 0 -- a rotational
+    discontinuity in the transverse velocity.
+    (a) With gamma = 3/2, P = 1/2, B_x = 2, u = 1/4 on both sides every intermediate is exact in binary
+    (gamma P = 3/4, discriminant 3.25^2, c_f = 2, S_M = 1/4) and D is 0.0 exactly: without the branch the
+    flux is NaN.  With it, the face sits between the two Alfven waves of a pure shear and the flux is the
+    closed form of that textbook problem (equal densities): v** = (v_L + v_R)/2,
+    B_t** = sgn(B_x) sqrt(rho) (v_R - v_L)/2, energy from the jump across the left Alfven wave.
+    (b) Whatever the branch does, the flux must be the limit of the regular formula: with
+    B_perp = delta (cos t, sin t) it converges linearly in delta to its value at delta = 0 through eight
+    decades, also with a 1e-9 or 1e-6 jump in u.  (A branch that drops the tangential velocity breaks this.)"""
+    g15, bx = 1.5, 2.0
+    WL = np.array([1.0, 0.25, 0.5, -0.25, 0.5, 0.0, 0.0])
+    WR = np.array([1.0, 0.25, -0.5, 0.75, 0.5, 0.0, 0.0])
+    F = orc.hlld(g15, WL, WR, bx)
+    assert np.all(np.isfinite(F))
+    # rotational discontinuity, rho = 1: between the Alfven waves v** = (v_L + v_R)/2 and
+    # B_t** = sqrt(rho) (v_R - v_L)/2 sgn(B_x) (M&K Eq. 59-62 with B_t = 0 outside)
+    vss, wss = 0.0, 0.25
+    byss, bzss = 0.5 * (-0.5 - 0.5), 0.5 * (0.75 + 0.25)
+    u = 0.25
+    pT = 0.5 + 0.5 * bx * bx
+    e_L = 0.5 / (g15 - 1.0) + 0.5 * (u * u + 0.25 + 0.0625) + 0.5 * bx * bx
+    # energy of the double-star state from the jump across the left Alfven wave (S*_L = u - 2)
+    ess = e_L - 1.0 * (u * bx + 0.0 - (u * bx + vss * byss + wss * bzss)) * 1.0
+    want = np.array([u, u * u + pT - bx * bx, u * vss - bx * byss, u * wss - bx * bzss,
+                     u * (ess + pT) - bx * (u * bx + vss * byss + wss * bzss), byss * u - bx * vss, bzss * u - bx * wss])
+    np.testing.assert_allclose(F, want, rtol=0, atol=1e-15)
+
+    th = 0.7
+
+    def flux(delta, du):
+        L = np.array([1.0, 0.3, 0.1, -0.2, 0.2, delta * np.cos(th), delta * np.sin(th)])
+        R = np.array([1.0, 0.3 + du, -0.3, 0.2, 0.2, delta * np.cos(th), delta * np.sin(th)])
+        return orc.hlld(G, L, R, bx)
+    for du in (0.0, 1e-9, 1e-6):
+        F0 = flux(0.0, du)
+        assert np.all(np.isfinite(F0))
+        for delta in (1e-2, 1e-4, 1e-6, 1e-8, 1e-10):
+            d = np.abs(flux(delta, du) - F0).max()
+            assert 1.0 * delta <= d <= 2.0 * delta, (du, delta, d)
+
+
 def test_T5_hlld_reduces_to_hllc_without_field():
     rng = np.random.default_rng(4)
     for it in range(500):
