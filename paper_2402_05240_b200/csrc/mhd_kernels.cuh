@@ -250,8 +250,10 @@ __device__ __forceinline__ void pcm_face(double (*st)[MHD_PRED_T], const State8 
 #ifndef MHD_MINB_UPD
 #define MHD_MINB_UPD 2
 #endif
+// (6 blocks = 40 registers spilled 16 B once the CFL rate's roots became cubic steps; 4 blocks, 60 registers:
+// 0.43 -> 0.40 ms at 256^3; 3 and 5 blocks 0.42, 0.40; 8 blocks 0.46)
 #ifndef MHD_MINB_UPDB
-#define MHD_MINB_UPDB 6
+#define MHD_MINB_UPDB 4
 #endif
 #ifndef MHD_MINB_CT
 #define MHD_MINB_CT 3
