@@ -492,6 +492,21 @@ __device__ __forceinline__ double select_(bool c, double a, double b) {
   return r;
 }
 
+// "D_f and the cell curvatures share a sign" on the sign bits (one LOP3 and one integer compare instead of a
+// fp64 multiply and a fp64 compare per curvature).  Zeros need no test of their own: with a zero among them
+// the limited curvature min(C |D|, |D_f|) is zero whichever way the test goes.
+#ifndef MHD_PPM_SIGN_INT
+#define MHD_PPM_SIGN_INT 1
+#endif
+__device__ __forceinline__ bool same_sign(double f, double a, double b) {
+  if (MHD_PPM_SIGN_INT) return ((hi32(f) ^ hi32(a)) | (hi32(f) ^ hi32(b))) >= 0;
+  return (f * a > 0.0) && (f * b > 0.0);
+}
+__device__ __forceinline__ bool same_sign(double f, double a, double b, double c) {
+  if (MHD_PPM_SIGN_INT) return ((hi32(f) ^ hi32(a)) | (hi32(f) ^ hi32(b)) | (hi32(f) ^ hi32(c))) >= 0;
+  return (f * a > 0.0) && (f * b > 0.0) && (f * c > 0.0);
+}
+
 __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, double qd) {
   const double C = 1.25;
   const double sbc = qb + qc;
@@ -499,7 +514,7 @@ __device__ __forceinline__ double ppm_face(double qa, double qb, double qc, doub
   const double Df = 3.0 * (qb - 2.0 * qf + qc);
   const double Dj = qa - 2.0 * qb + qc;
   const double Dj1 = qb - 2.0 * qc + qd;
-  const bool same = (Df * Dj > 0.0) && (Df * Dj1 > 0.0);
+  const bool same = same_sign(Df, Dj, Dj1);
   const double Dlim = select_(same, copysign(amin_(C * amin_(Dj, Dj1), Df), Df), 0.0);
   const double qlim = 0.5 * sbc - Dlim * (1.0 / 6.0);
   return ((qf - qb) * (qc - qf) < 0.0) ? qlim : qf;
@@ -514,17 +529,20 @@ __device__ __forceinline__ void ppm_scalar(double q0, double q1, double q2, doub
   // reading R7: differences that are zero to round-off count as zero in the extremum test
   const double tau = 1e-12 * fabs(amax_(q1, amax_(q2, q3)));
   double dm = qi - qm, dp = qp - qi, e3 = q3 - qi, e1 = qi - q1;
-  dm = (fabs(dm) <= tau) ? 0.0 : dm;
-  dp = (fabs(dp) <= tau) ? 0.0 : dp;
-  e3 = (fabs(e3) <= tau) ? 0.0 : e3;
-  e1 = (fabs(e1) <= tau) ? 0.0 : e1;
-  const bool extremum = (dm * dp <= 0.0) || (e3 * e1 <= 0.0);
+  const bool zm = fabs(dm) <= tau, zp = fabs(dp) <= tau, z3 = fabs(e3) <= tau, z1 = fabs(e1) <= tau;
+  dm = zm ? 0.0 : dm;
+  dp = zp ? 0.0 : dp;
+  // "dm dp <= 0 or e3 e1 <= 0": a flushed difference, or a pair of opposite sign (the flush predicates are
+  // the zero tests; the sign bits of the unflushed differences do the rest)
+  const bool extremum = MHD_PPM_SIGN_INT
+                            ? (zm || zp || z3 || z1 || ((hi32(dm) ^ hi32(dp)) | (hi32(e3) ^ hi32(e1))) < 0)
+                            : (dm * dp <= 0.0) || ((z3 ? 0.0 : e3) * (z1 ? 0.0 : e1) <= 0.0);
   // at an extremum: the parabola's curvature limited against the cell curvatures
   const double Df = 6.0 * (qm - 2.0 * qi + qp);
   const double Dm1 = q0 - 2.0 * q1 + q2;
   const double D0 = q1 - 2.0 * q2 + q3;
   const double Dp1 = q2 - 2.0 * q3 + q4;
-  const bool same = (Df * Dm1 > 0.0) && (Df * D0 > 0.0) && (Df * Dp1 > 0.0);
+  const bool same = same_sign(Df, Dm1, D0, Dp1);
   const double Dlim = select_(same, copysign(amin_(C * amin_(Dm1, amin_(D0, Dp1)), Df), Df), 0.0);
   const bool big = fabs(Df) > max_(tau, 1e-290);          // (the floor keeps rcp off denormals)
   const double r = big ? Dlim * rcp(big ? Df : 1.0) : 0.0;
