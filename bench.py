@@ -60,7 +60,7 @@ NCU_TRAFFIC_GB = {1: {"k_predictor_stage": 2.78, "k_flux_x": 2.07, "k_flux_march
 STEP_FLOP_PER_CELL = sum(v[0] for v in KERNEL_MODEL.values())     # 4310 (PLMC; PPMC 4900), algorithmic
 # what this build executes per active cell and step (ncu, profiles/r2_ncu_kernels.md): flop = dadd + dmul +
 # 2 dfma summed over the step's kernels (halo columns of the stage kernel included); DRAM bytes read + written
-EXECUTED_FLOP_PER_CELL = {1: 3598, 2: 5194}   # (the branch-free PPM limiter evaluates every candidate value)
+EXECUTED_FLOP_PER_CELL = {1: 3598, 2: 4993}   # (the branch-free PPM limiter evaluates every candidate value)
 NCU_STEP_DRAM_BYTES_PER_CELL = {1: 918, 2: 948}
 
 
